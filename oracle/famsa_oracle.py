@@ -1,0 +1,135 @@
+"""Python face of the CPU oracle -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this.  It imports nothing from paper_1603_06958_b200 (the CUDA path)
+and the CUDA path imports nothing from here.
+
+What it computes (arxiv 1603.06958, readings in DESIGN.md):
+  encode      residue bytes -> 25-letter codes                       (R9, R10)
+  sort_perm   descending length, ties by ascending original index    (R15)
+  lcs_len     textbook DP LCS length
+  indel       |A| + |B| - 2 LCS
+  similarity  LCS / indel^2 in float64
+  rows        the packed-triangular row block [i0, i1) in sorted index space:
+              entry (i, j<i) at i(i-1)/2 - i0(i0-1)/2 + j            (R16)
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(_build.build())
+        u8p = ctypes.POINTER(ctypes.c_uint8)
+        i64p = ctypes.POINTER(ctypes.c_int64)
+        lib.oracle_encode.restype = ctypes.c_int64
+        lib.oracle_encode.argtypes = [u8p, ctypes.c_int64, u8p]
+        lib.oracle_lcs_len.restype = ctypes.c_int32
+        lib.oracle_lcs_len.argtypes = [u8p, ctypes.c_int32, u8p, ctypes.c_int32]
+        lib.oracle_indel.restype = ctypes.c_int64
+        lib.oracle_indel.argtypes = [ctypes.c_int64] * 3
+        lib.oracle_similarity.restype = ctypes.c_double
+        lib.oracle_similarity.argtypes = [ctypes.c_int64] * 3
+        lib.oracle_pairs.restype = ctypes.c_int
+        lib.oracle_pairs.argtypes = [u8p, i64p, i64p, i64p, ctypes.c_int64,
+                                     ctypes.POINTER(ctypes.c_int32),
+                                     ctypes.POINTER(ctypes.c_double), ctypes.c_int32]
+        _lib = lib
+    return _lib
+
+
+def _u8(a):
+    a = np.ascontiguousarray(a, dtype=np.uint8)
+    return a, a.ctypes.data_as(ctypes.POINTER(ctypes.c_uint8))
+
+
+def _i64(a):
+    a = np.ascontiguousarray(a, dtype=np.int64)
+    return a, a.ctypes.data_as(ctypes.POINTER(ctypes.c_int64))
+
+
+def as_bytes(seq):
+    """str / bytes / array -> uint8 array (no encoding)."""
+    if isinstance(seq, str):
+        seq = seq.encode("ascii")
+    if isinstance(seq, (bytes, bytearray)):
+        return np.frombuffer(bytes(seq), dtype=np.uint8).copy()
+    return np.ascontiguousarray(seq, dtype=np.uint8)
+
+
+def encode(seq):
+    """Residue bytes -> codes 0..24.  Raises ValueError at the first bad symbol."""
+    raw, rp = _u8(as_bytes(seq))
+    out = np.empty_like(raw)
+    bad = _load().oracle_encode(rp, raw.size, out.ctypes.data_as(ctypes.POINTER(ctypes.c_uint8)))
+    if bad >= 0:
+        raise ValueError("bad residue byte %d at position %d" % (int(raw[bad]), bad))
+    return out
+
+
+def lcs_len(a, b):
+    """LCS length of two sequences (encoded first, so 'a' == 'A' == code 0)."""
+    ea, pa = _u8(encode(a))
+    eb, pb = _u8(encode(b))
+    return int(_load().oracle_lcs_len(pa, ea.size, pb, eb.size))
+
+
+def indel(la, lb, lcs):
+    return int(_load().oracle_indel(int(la), int(lb), int(lcs)))
+
+
+def similarity(la, lb, lcs):
+    return float(_load().oracle_similarity(int(la), int(lb), int(lcs)))
+
+
+def sort_perm(offsets):
+    """perm[sorted] = original index: descending length, ties by ascending index (R15)."""
+    offsets = np.asarray(offsets, dtype=np.int64)
+    lens = np.diff(offsets)
+    return np.argsort(-lens, kind="stable").astype(np.int64)
+
+
+def n_threads_default():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def pairs(seqs, offsets, pi, pj, want_sim=True, n_threads=None):
+    """LCS (int32) and similarity (float64) for pairs (pi[p], pj[p]) in ORIGINAL index space."""
+    codes, cp = _u8(encode(seqs))
+    offsets, op = _i64(offsets)
+    pi, pip = _i64(pi)
+    pj, pjp = _i64(pj)
+    n = pi.size
+    lcs = np.empty(n, dtype=np.int32)
+    sim = np.empty(n, dtype=np.float64) if want_sim else None
+    if n_threads is None:
+        n_threads = n_threads_default()
+    _load().oracle_pairs(cp, op, pip, pjp, n,
+                         lcs.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
+                         sim.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if want_sim else None,
+                         int(n_threads))
+    return lcs, sim
+
+
+def rows_pairs(i0, i1):
+    """Number of entries of row block [i0, i1): sum_{i=i0}^{i1-1} i."""
+    return i1 * (i1 - 1) // 2 - i0 * (i0 - 1) // 2
+
+
+def rows(seqs, offsets, i0, i1, want_sim=True, n_threads=None):
+    """Row block [i0, i1) in SORTED index space, packed triangular by rows (R16)."""
+    perm = sort_perm(offsets)
+    ii = np.repeat(np.arange(i0, i1, dtype=np.int64), np.arange(i0, i1, dtype=np.int64))
+    row_start = ii * (ii - 1) // 2 - i0 * (i0 - 1) // 2
+    jj = np.arange(ii.size, dtype=np.int64) - row_start
+    return pairs(seqs, offsets, perm[ii], perm[jj], want_sim, n_threads)
