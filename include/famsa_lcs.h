@@ -1,0 +1,133 @@
+/*
+ * famsa_lcs.h -- C-ABI boundary of the B200-native FAMSA stage I hot path
+ * (arxiv 1603.06958, "Pairwise similarities calculation"):
+ * all-pairs LCS length (bit-parallel), indel distance
+ * and similarity = LCS / indel^2, streamed in row blocks so that the
+ * single-linkage consumer needs O(k) memory.
+ *
+ * Plain pointers and sizes only; each pointer is marked HOST or DEVICE.  No exception
+ * crosses the ABI.  Every int-returning call returns 0 (FAMSA_OK) or a negative
+ * FAMSA_E* code; famsa_last_error() gives the text for the calling thread.
+ * There is NO CPU fallback: without an sm_100 CUDA device famsa_pack fails with
+ * FAMSA_ECUDA.
+ *
+ * Index space.  famsa_pack sorts sequences by DESCENDING length, ties by ascending
+ * original index (stable).  All row/column indices below are SORTED indices;
+ * famsa_perm maps sorted -> original.  Row i holds pairs (i, j) for 0 <= j < i; in each
+ * such pair sequence i is the shorter one and carries the bit-vectors (LCS is symmetric).
+ *
+ * Output layout.  For a call over rows [i0, i1): entry (i, j) is at
+ *     i*(i-1)/2 - i0*(i0-1)/2 + j
+ * in both lcs_out and sim_out (two arrays, packed triangular by rows; row i contiguous).
+ */
+#ifndef FAMSA_LCS_H
+#define FAMSA_LCS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct famsa_ctx famsa_ctx;   /* opaque; owns every device allocation it makes */
+
+enum {
+    FAMSA_OK      = 0,
+    FAMSA_EINVAL  = -1,  /* null pointer, k < 0, offsets[0] != 0 or offsets decreasing     */
+    FAMSA_ESYMBOL = -2,  /* a byte that is neither a code (< 25) nor an amino-acid letter  */
+    FAMSA_ELENGTH = -3,  /* an empty sequence, or one longer than FAMSA_MAX_LEN            */
+    FAMSA_ERANGE  = -4,  /* i0 > i1, i0 < 0 or i1 > k                                      */
+    FAMSA_ENOMEM  = -5,  /* host or device allocation failed                               */
+    FAMSA_ECUDA   = -6   /* any CUDA runtime error, or no sm_100 device                    */
+};
+
+#define FAMSA_MAX_LEN 65535   /* so that every LCS length fits uint16 */
+
+/*
+ * famsa_pack -- steps a1-a3 of the path (encode, length sort, match-table build); one-off,
+ * O(sum |S|), runs on the device.
+ *   seqs     HOST  concatenated residues, no terminators.  A byte < 25 is already a code;
+ *                  ASCII letters (either case) map to the 25-letter code
+ *                  ACDEFGHIKLMNPQRSTVWY + B Z X U O (J -> X).  Anything else: FAMSA_ESYMBOL.
+ *   offsets  HOST  k+1 entries, offsets[0] = 0, sequence s = seqs[offsets[s], offsets[s+1]).
+ *   k        number of sequences (0 and 1 are legal: zero pairs).
+ *   device   CUDA device ordinal to pack onto (the ctx stays bound to it).
+ *   out      receives the handle.  Inputs are copied; the caller may free them on return.
+ * Builds, per sequence S and symbol c, the match bit-vectors M_S[c] (bit i set iff
+ * S[i] == c; "bit-parallel approach") and the pre-scaled, lane-interleaved
+ * residue streams the sweep reads.  Synchronises the device before returning.
+ */
+int famsa_pack(const uint8_t* seqs, const int64_t* offsets, int64_t k, int device,
+               famsa_ctx** out);
+
+/*
+ * famsa_lcs_rows -- steps a4-a7: the pair sweep for rows [i0, i1), all columns j < i.
+ * For each pair, with A = sequence i (shorter) and B = sequence j: V <- all ones; for each
+ * residue b of B: U = V & M_A[b]; V = (V + U) | (V - U) with the add carry propagated across
+ * words; LCS = number of zero bits of V (recurrence as stated in BASELINE.json
+ * north_star).  Then indel = |A| + |B| - 2 LCS and
+ * similarity = LCS / indel^2 in fp32 (+inf when indel = 0).
+ *   lcs_out  DEVICE  famsa_rows_pairs(i0, i1) uint16 entries, layout above.  May be NULL
+ *                    only if sim_out is not.
+ *   sim_out  DEVICE  same count of float entries, or NULL (LCS only).
+ *   cuda_stream      a cudaStream_t (NULL = default stream).  Work is ENQUEUED, not
+ *                    synchronised; the buffers belong to the caller and must stay valid
+ *                    until the stream has run.  One ctx may serve concurrent calls on
+ *                    different streams (it is read-only after pack).
+ * Errors: FAMSA_EINVAL (null ctx, both outputs NULL), FAMSA_ERANGE, FAMSA_ECUDA.
+ */
+int famsa_lcs_rows(famsa_ctx* ctx, int64_t i0, int64_t i1,
+                   uint16_t* lcs_out, float* sim_out, void* cuda_stream);
+
+/*
+ * famsa_lcs_rows_host -- the same call for HOST output buffers (the end-to-end path):
+ * sweeps rows [i0, i1) in row blocks on the device and copies each block back, device
+ * compute overlapped with the device->host copy of the previous block.  Synchronous.
+ *   lcs_host, sim_host  HOST  as above (either may be NULL, not both); pageable or pinned.
+ */
+int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1,
+                        uint16_t* lcs_host, float* sim_host);
+
+/* Number of (i, j < i) entries of rows [i0, i1): i1(i1-1)/2 - i0(i0-1)/2.  -1 if i0 > i1 or i0 < 0. */
+int64_t famsa_rows_pairs(int64_t i0, int64_t i1);
+
+/* True DP cells of rows [i0, i1): sum over pairs of |A|*|B| (what GCUPS counts; padding excluded). */
+int famsa_rows_cells(const famsa_ctx* ctx, int64_t i0, int64_t i1, double* cells);
+
+int famsa_k(const famsa_ctx* ctx, int64_t* k);
+int famsa_perm(const famsa_ctx* ctx, int64_t* perm_host);      /* HOST, k entries: perm[sorted] = original */
+int famsa_lengths(const famsa_ctx* ctx, uint32_t* len_host);   /* HOST, k entries, sorted order            */
+
+/*
+ * Introspection of what pack built (tests): decoded residues and match-table words.
+ *   famsa_codes   HOST out, len entries: codes 0..24 of sorted sequence s, read back from the
+ *                 device-resident interleaved stream.
+ *   famsa_match   HOST out, ceil(len/32) words: M_s[c] read back from the device table.
+ */
+int famsa_codes(const famsa_ctx* ctx, int64_t s, uint8_t* codes_host);
+int famsa_match(const famsa_ctx* ctx, int64_t s, int c, uint32_t* words_host);
+
+/* Kernel launches enqueued by this ctx so far (pack + sweep), for bench.py's gpu_launches. */
+int64_t famsa_launch_count(const famsa_ctx* ctx);
+
+/*
+ * famsa_alu_peak -- micro-benchmark that measures the chip's INT32 ALU-pipe issue rate
+ * (independent LOP3/IADD3 chains, all SMs, full occupancy): the roofline denominator.
+ *   device            CUDA device ordinal
+ *   instr_per_s       HOST out: warp-lane INT32 instructions per second (thread-instr/s)
+ *   instr_per_clk_sm  HOST out: the same per SM per clock, using sm_mhz below
+ *   sm_mhz            HOST out: SM clock achieved during the run (clock64 / elapsed time)
+ */
+int famsa_alu_peak(int device, double* instr_per_s, double* instr_per_clk_sm, double* sm_mhz);
+
+/* Tuning knob (process-wide, tests sweep it): rows of A per CTA on the register path, 1..12. */
+int famsa_set_tuning(int rows_per_cta);
+
+void famsa_free(famsa_ctx* ctx);            /* famsa_free(NULL) is a no-op */
+const char* famsa_strerror(int code);       /* static text for a FAMSA_E* code */
+const char* famsa_last_error(void);         /* detail of the calling thread's last failure */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FAMSA_LCS_H */

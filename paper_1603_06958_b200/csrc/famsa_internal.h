@@ -1,0 +1,88 @@
+// famsa_internal.h -- shared between the translation units of libfamsa_lcs.so (CUDA path only;
+// nothing under oracle/ includes this).  Device data layout of a packed sequence set.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <atomic>
+#include <string>
+#include <vector>
+
+#include "famsa_lcs.h"
+
+namespace famsa {
+
+// ---- layout constants ---------------------------------------------------------------------
+// Residue stream ("B side"): sorted sequences in groups of 32 (one group = the 32 lanes of a
+// warp), 16-byte chunks interleaved by lane: byte p of lane l of group g sits at
+//     stream[(goff[g] + p/16) * 512 + l*16 + p%16].
+// Each byte is code*4 (the byte offset of the symbol inside a 128-byte table row); positions
+// past the end of a sequence hold PAD_BYTE, whose table row (symbol 31) is all-zero, so a pad
+// residue leaves V unchanged.
+constexpr int      GROUP      = 32;
+constexpr int      CHUNK      = 16;
+constexpr uint8_t  PAD_BYTE   = 31 * 4;
+// Match tables ("A side"): per sequence, words x 32 symbols, layout [word][symbol] uint32, so a
+// warp reading one word for 32 different residues touches one 128-byte row (bank = symbol).
+// A sequence of Ws = ceil(len/32) words is cut into nblk blocks of Wb <= 32 words; each block is
+// stored with an even word stride Wst so every block base is 256-byte aligned.
+constexpr int      SYMS       = 32;
+constexpr int      ROW_BYTES  = SYMS * 4;       // 128
+constexpr int      MAX_WB     = 32;             // V words held in registers per thread
+constexpr int      CW_SMALL   = 128;            // carry-vector words (long path), |B| <= 4096
+constexpr int      CW_LARGE   = 2048;           // |B| <= 65535
+
+struct BlockPlan { int nblk; int wb; int wst; };   // wst = wb rounded up to even
+
+inline BlockPlan plan_blocks(uint32_t len, bool force32) {
+    int ws = (int)((len + 31) / 32);
+    BlockPlan p;
+    p.nblk = (ws + MAX_WB - 1) / MAX_WB;
+    p.wb = (p.nblk > 1 && force32) ? MAX_WB : (ws + p.nblk - 1) / p.nblk;
+    p.wst = (p.wb + 1) & ~1;
+    return p;
+}
+
+struct Bucket { int64_t r0, r1; int nblk, wb; };   // rows [r0, r1) share one kernel variant
+
+}  // namespace famsa
+
+struct famsa_ctx {
+    int      device = 0;
+    int      sm_count = 0;
+    int64_t  k = 0;
+    int64_t  n_groups = 0;
+    uint32_t max_len = 0;
+    bool     large_cw = false;                  // some sequence longer than 4096
+    // host copies
+    std::vector<int64_t>  perm;                 // perm[sorted] = original
+    std::vector<uint32_t> len;                  // sorted order
+    std::vector<uint32_t> toff;                 // table offset of sorted sequence s, in 128-byte rows
+    std::vector<uint32_t> goff;                 // n_groups+1: stream offset of group g, in 512-byte units
+    std::vector<double>   len_prefix;           // k+1: sum of len[0..s)
+    std::vector<famsa::Bucket> buckets;
+    // device
+    uint8_t*  d_stream = nullptr;  size_t stream_bytes = 0;
+    uint32_t* d_tables = nullptr;  size_t table_bytes = 0;
+    uint32_t* d_len = nullptr;
+    uint32_t* d_toff = nullptr;
+    uint32_t* d_goff = nullptr;
+    // row-block staging for famsa_lcs_rows_host (lazily allocated)
+    uint16_t* d_lcs_buf[2] = {nullptr, nullptr};
+    float*    d_sim_buf[2] = {nullptr, nullptr};
+    size_t    buf_pairs = 0;
+    cudaStream_t s_compute = nullptr, s_copy = nullptr;
+    cudaEvent_t  ev_done[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
+    std::atomic<int64_t> launches{0};
+};
+
+namespace famsa {
+void set_error(const std::string& msg);
+int  cuda_fail(cudaError_t e, const char* what);          // records text, returns FAMSA_ECUDA
+int  sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim, cudaStream_t st);
+}  // namespace famsa
+
+#define FAMSA_CUDA(call)                                                     \
+    do {                                                                     \
+        cudaError_t e__ = (call);                                            \
+        if (e__ != cudaSuccess) return famsa::cuda_fail(e__, #call);         \
+    } while (0)

@@ -1,0 +1,333 @@
+// famsa_sweep.cu -- steps a4-a7 of the path: the all-pairs bit-parallel LCS sweep, zero count,
+// similarity epilogue and packed-triangular row store (recurrence as
+// stated in BASELINE.json north_star, cited by the paper as Hyyro [15]).
+//
+// Mapping: one thread = one pair at a time.  A CTA owns TA rows (A side:
+// match tables staged in shared memory, layout [word][symbol] so one warp load = one 128-byte
+// row, no bank conflict for any residue mix) x TB columns (B side: thread t walks sequence
+// j0 + t; a warp = one 32-lane interleave group, so each uint4 load is 512 contiguous bytes).
+// V lives in W registers; the add carry runs through the hardware carry flag
+// (add.cc / addc.cc -> IADD3 / IADD3.X).  Per 32-bit word-step: LOP3, IADD3.X, LOP3 + one LDS.
+// Rows longer than 32 words are cut into blocks of Wb <= 32 words; the carry out of block t at
+// residue p is kept in a per-thread bit-vector and fed to block t+1 at residue p.
+#include <algorithm>
+
+#include "famsa_internal.h"
+
+namespace famsa {
+
+constexpr int TB = 128;          // threads (= columns) per CTA
+constexpr int MAX_ROWS_PER_LAUNCH = 1024;
+
+struct SweepArgs {
+    const uint4*    stream;      // interleaved residue stream
+    const uint32_t* goff;        // group offsets (512-byte units)
+    const uint4*    tables;      // match tables, 128-byte rows
+    const uint32_t* toff;        // table row offset per sequence
+    const uint32_t* len;         // lengths, sorted order
+    uint16_t*       lcs_out;
+    float*          sim_out;
+    int64_t         out_base;    // i0*(i0-1)/2 of the call
+    uint32_t        r0, r1;      // rows of this launch
+    uint32_t        ta;          // rows per CTA
+    uint32_t        n_col_tiles;
+    uint32_t        nblk;        // table blocks per row (1 on the register path)
+};
+
+template <int IMM>
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+    uint32_t v;
+    asm("ld.shared.u32 %0, [%1+%2];" : "=r"(v) : "r"(addr), "n"(IMM));
+    return v;
+}
+// m[w] = table word w of the symbol column at `addr` (static unroll so the offset is an immediate)
+template <int W, int I = 0>
+struct LoadWords {
+    static __device__ __forceinline__ void run(uint32_t (&m)[W], uint32_t addr) {
+        m[I] = lds32<I * ROW_BYTES>(addr);
+        LoadWords<W, I + 1>::run(m, addr);
+    }
+};
+template <int W>
+struct LoadWords<W, W> {
+    static __device__ __forceinline__ void run(uint32_t (&)[W], uint32_t) {}
+};
+
+// One residue against W words of V.  `addr` = shared-memory address of the symbol's column in
+// word-row 0 (table base | code*4).  CARRY: the chain starts from / ends in the hardware carry.
+template <int W, bool CARRY>
+__device__ __forceinline__ void residue_step(uint32_t (&V)[W], uint32_t addr, uint32_t& cin, uint32_t& cout) {
+    uint32_t m[W], s[W];
+    LoadWords<W>::run(m, addr);
+    if (CARRY) asm volatile("add.cc.u32 %0, %0, %0;" : "+r"(cin));            // carry flag <- top bit of cin
+#pragma unroll
+    for (int w = 0; w < W; ++w) {
+        uint32_t u = V[w] & m[w];
+        if (w == 0 && !CARRY) asm volatile("add.cc.u32 %0, %1, %2;" : "=r"(s[w]) : "r"(V[w]), "r"(u));
+        else                  asm volatile("addc.cc.u32 %0, %1, %2;" : "=r"(s[w]) : "r"(V[w]), "r"(u));
+    }
+    if (CARRY) asm volatile("addc.u32 %0, %0, %0;" : "+r"(cout));             // shift the carry out in
+#pragma unroll
+    for (int w = 0; w < W; ++w) V[w] = s[w] | (V[w] & ~m[w]);
+}
+
+template <int W, bool CARRY>
+__device__ __forceinline__ void word_step(uint32_t (&V)[W], uint32_t bword, uint32_t tbase, uint32_t& cin, uint32_t& cout) {
+    // byte r of bword is code*4 (< 128); tbase is 256-byte aligned, so PRMT splices the byte in.
+    residue_step<W, CARRY>(V, __byte_perm(bword, tbase, 0x7650), cin, cout);
+    residue_step<W, CARRY>(V, __byte_perm(bword, tbase, 0x7651), cin, cout);
+    residue_step<W, CARRY>(V, __byte_perm(bword, tbase, 0x7652), cin, cout);
+    residue_step<W, CARRY>(V, __byte_perm(bword, tbase, 0x7653), cin, cout);
+}
+
+// Sweep all chunks of this warp's group against one table block.  cv: carry bit-vector (16 bits
+// per chunk) or nullptr-equivalent when !CARRY.
+template <int W, bool CARRY>
+__device__ __forceinline__ void sweep_block(uint32_t (&V)[W], const uint4* __restrict__ bp, uint32_t nch, uint32_t tbase,
+                                            unsigned short* cv, bool read_cv, bool write_cv) {
+    uint4 cur = nch ? __ldg(bp) : make_uint4(0, 0, 0, 0);
+    for (uint32_t c = 0; c < nch; ++c) {
+        uint4 nxt = cur;
+        if (c + 1 < nch) nxt = __ldg(bp + (size_t)(c + 1) * GROUP);
+        uint32_t cin = 0, cout = 0;
+        if (CARRY && read_cv) cin = (uint32_t)cv[c] << 16;
+        word_step<W, CARRY>(V, cur.x, tbase, cin, cout);
+        word_step<W, CARRY>(V, cur.y, tbase, cin, cout);
+        word_step<W, CARRY>(V, cur.z, tbase, cin, cout);
+        word_step<W, CARRY>(V, cur.w, tbase, cin, cout);
+        if (CARRY && write_cv) cv[c] = (unsigned short)cout;
+        cur = nxt;
+    }
+}
+
+__device__ __forceinline__ void store_pair(const SweepArgs& a, uint32_t i, uint32_t j, uint32_t la, uint32_t lb, uint32_t lcs) {
+    int64_t pos = (int64_t)i * (i - 1) / 2 - a.out_base + j;
+    if (a.lcs_out) a.lcs_out[pos] = (unsigned short)lcs;
+    if (a.sim_out) {
+        // indel = |A| + |B| - 2 LCS; similarity = LCS / indel^2
+        unsigned long long indel = (unsigned long long)la + lb - 2ull * lcs;
+        a.sim_out[pos] = __fdiv_rn(__uint2float_rn(lcs), __ull2float_rn(indel * indel));
+    }
+}
+
+// ---- register path: every row of the launch fits one block of W words --------------------------
+template <int W>
+__global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
+    extern __shared__ __align__(256) uint8_t smem[];
+    constexpr int WST = (W + 1) & ~1;
+    const uint32_t col_tile = blockIdx.x % a.n_col_tiles, row_tile = blockIdx.x / a.n_col_tiles;
+    const uint32_t r_lo = a.r0 + row_tile * a.ta;
+    const uint32_t r_hi = min(r_lo + a.ta, a.r1);
+    const uint32_t j0 = col_tile * TB;
+    if (j0 + 1 >= r_hi) return;                          // whole tile on or above the diagonal
+    // stage the tile's tables: rows r_lo..r_hi-1 are contiguous (same stride WST each)
+    {
+        const uint4* src = a.tables + (size_t)a.toff[r_lo] * (ROW_BYTES / 16);
+        uint4* dst = reinterpret_cast<uint4*>(smem);
+        const uint32_t n16 = (r_hi - r_lo) * WST * (ROW_BYTES / 16);
+        for (uint32_t t = threadIdx.x; t < n16; t += TB) dst[t] = __ldg(src + t);
+    }
+    __syncthreads();
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t jw = j0 + (threadIdx.x & ~31u);       // first column of this warp
+    if (jw + 1 >= r_hi) return;                          // this warp's columns are all >= every row (no barrier follows)
+    const uint32_t j = jw + lane;
+    const uint32_t g = jw / GROUP;                       // jw < k, so g is a real group
+    const uint32_t gb = a.goff[g], nch = a.goff[g + 1] - gb;
+    const uint4* bp = a.stream + (size_t)gb * GROUP + lane;
+    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t lb = j < r_hi ? a.len[j] : 0;         // columns >= r_hi are never stored
+    for (uint32_t i = max(r_lo, jw + 1); i < r_hi; ++i) {
+        uint32_t V[W];
+#pragma unroll
+        for (int w = 0; w < W; ++w) V[w] = 0xFFFFFFFFu;
+        sweep_block<W, false>(V, bp, nch, smem_base + (i - r_lo) * (WST * ROW_BYTES), nullptr, false, false);
+        uint32_t lcs = 0;
+#pragma unroll
+        for (int w = 0; w < W; ++w) lcs += __popc(~V[w]);
+        if (j < i) store_pair(a, i, j, a.len[i], lb, lcs);
+    }
+}
+
+// ---- blocked path: rows of nblk blocks x W words; one row per CTA; carry bit-vector per thread --
+template <int W, int CW>
+__global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
+    extern __shared__ __align__(256) uint8_t smem[];
+    constexpr int WST = (W + 1) & ~1;
+    const uint32_t col_tile = blockIdx.x % a.n_col_tiles, row_tile = blockIdx.x / a.n_col_tiles;
+    const uint32_t i = a.r0 + row_tile;
+    const uint32_t j0 = col_tile * TB;
+    if (j0 >= i) return;
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t jw = j0 + (threadIdx.x & ~31u);
+    const uint32_t j = jw + lane;
+    const bool active = jw < i;                          // warp-uniform
+    uint32_t gb = 0, nch = 0;
+    if (active) { const uint32_t g = jw / GROUP; gb = a.goff[g]; nch = a.goff[g + 1] - gb; }
+    const uint4* bp = a.stream + (size_t)gb * GROUP + lane;
+    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+    unsigned short cv[CW * 2];                           // 16 carry bits per 16-residue chunk
+    uint32_t lcs = 0;
+    const uint4* src = a.tables + (size_t)a.toff[i] * (ROW_BYTES / 16);
+    for (uint32_t blk = 0; blk < a.nblk; ++blk) {
+        if (blk) __syncthreads();                        // everyone done with the previous block
+        uint4* dst = reinterpret_cast<uint4*>(smem);
+        for (uint32_t t = threadIdx.x; t < WST * (ROW_BYTES / 16); t += TB)
+            dst[t] = __ldg(src + (size_t)blk * WST * (ROW_BYTES / 16) + t);
+        __syncthreads();
+        if (active) {
+            uint32_t V[W];
+#pragma unroll
+            for (int w = 0; w < W; ++w) V[w] = 0xFFFFFFFFu;
+            sweep_block<W, true>(V, bp, nch, smem_base, cv, blk > 0, blk + 1 < a.nblk);
+#pragma unroll
+            for (int w = 0; w < W; ++w) lcs += __popc(~V[w]);
+        }
+    }
+    if (active && j < i) store_pair(a, i, j, a.len[i], a.len[j], lcs);
+}
+
+}  // namespace famsa
+
+// ---- host side: buckets -> launches ------------------------------------------------------------
+namespace famsa {
+
+template <int W>
+static cudaError_t launch_short(const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st) {
+    sweep_short_kernel<W><<<grid, TB, smem, st>>>(a);
+    return cudaGetLastError();
+}
+template <int W, int CW>
+static cudaError_t launch_long(const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st) {
+    sweep_long_kernel<W, CW><<<grid, TB, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+#define SHORT_CASE(W) case W: return launch_short<W>(a, grid, smem, st);
+static cudaError_t dispatch_short(int w, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st) {
+    switch (w) {
+        SHORT_CASE(1) SHORT_CASE(2) SHORT_CASE(3) SHORT_CASE(4) SHORT_CASE(5) SHORT_CASE(6) SHORT_CASE(7) SHORT_CASE(8)
+        SHORT_CASE(9) SHORT_CASE(10) SHORT_CASE(11) SHORT_CASE(12) SHORT_CASE(13) SHORT_CASE(14) SHORT_CASE(15) SHORT_CASE(16)
+        SHORT_CASE(17) SHORT_CASE(18) SHORT_CASE(19) SHORT_CASE(20) SHORT_CASE(21) SHORT_CASE(22) SHORT_CASE(23) SHORT_CASE(24)
+        SHORT_CASE(25) SHORT_CASE(26) SHORT_CASE(27) SHORT_CASE(28) SHORT_CASE(29) SHORT_CASE(30) SHORT_CASE(31) SHORT_CASE(32)
+        default: return cudaErrorInvalidValue;
+    }
+}
+#define LONG_CASE(W) case W: return launch_long<W, CW_SMALL>(a, grid, smem, st);
+static cudaError_t dispatch_long(int w, bool large, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st) {
+    if (large) return w == 32 ? launch_long<32, CW_LARGE>(a, grid, smem, st) : cudaErrorInvalidValue;
+    switch (w) {
+        LONG_CASE(17) LONG_CASE(18) LONG_CASE(19) LONG_CASE(20) LONG_CASE(21) LONG_CASE(22) LONG_CASE(23) LONG_CASE(24)
+        LONG_CASE(25) LONG_CASE(26) LONG_CASE(27) LONG_CASE(28) LONG_CASE(29) LONG_CASE(30) LONG_CASE(31) LONG_CASE(32)
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+static uint32_t g_rows_per_cta = 8;     // TA; tunable through famsa_set_tuning (tests sweep it)
+
+int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim, cudaStream_t st) {
+    SweepArgs a;
+    a.stream = reinterpret_cast<const uint4*>(ctx->d_stream);
+    a.goff = ctx->d_goff;
+    a.tables = reinterpret_cast<const uint4*>(ctx->d_tables);
+    a.toff = ctx->d_toff;
+    a.len = ctx->d_len;
+    a.lcs_out = lcs; a.sim_out = sim;
+    a.out_base = i0 * (i0 - 1) / 2;
+    for (const Bucket& b : ctx->buckets) {
+        int64_t lo = std::max(b.r0, std::max<int64_t>(i0, 1)), hi = std::min(b.r1, i1);   // row 0 is empty
+        for (int64_t r = lo; r < hi; r += MAX_ROWS_PER_LAUNCH) {
+            a.r0 = (uint32_t)r; a.r1 = (uint32_t)std::min<int64_t>(r + MAX_ROWS_PER_LAUNCH, hi);
+            a.nblk = (uint32_t)b.nblk;
+            a.n_col_tiles = (a.r1 - 1 + TB - 1) / TB;                // columns 0 .. r1-2
+            const int wst = (b.wb + 1) & ~1;
+            cudaError_t e;
+            if (b.nblk == 1) {
+                a.ta = g_rows_per_cta;
+                unsigned row_tiles = (a.r1 - a.r0 + a.ta - 1) / a.ta;
+                e = dispatch_short(b.wb, a, row_tiles * a.n_col_tiles, (size_t)a.ta * wst * ROW_BYTES, st);
+            } else {
+                a.ta = 1;
+                e = dispatch_long(b.wb, ctx->large_cw, a, (a.r1 - a.r0) * a.n_col_tiles, (size_t)wst * ROW_BYTES, st);
+            }
+            if (e != cudaSuccess) return cuda_fail(e, "sweep kernel launch");
+            ctx->launches++;
+        }
+    }
+    return FAMSA_OK;
+}
+
+}  // namespace famsa
+
+using namespace famsa;
+
+extern "C" int famsa_set_tuning(int rows_per_cta) {
+    if (rows_per_cta < 1 || rows_per_cta > 12) { set_error("famsa_set_tuning: rows_per_cta must be 1..12"); return FAMSA_EINVAL; }
+    g_rows_per_cta = (uint32_t)rows_per_cta;
+    return FAMSA_OK;
+}
+
+extern "C" int famsa_lcs_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_out, float* sim_out,
+                              void* cuda_stream) {
+    if (!ctx) { set_error("famsa_lcs_rows: ctx is NULL"); return FAMSA_EINVAL; }
+    if (i0 < 0 || i0 > i1 || i1 > ctx->k) { set_error("famsa_lcs_rows: bad row range"); return FAMSA_ERANGE; }
+    if (!lcs_out && !sim_out) { set_error("famsa_lcs_rows: both outputs are NULL"); return FAMSA_EINVAL; }
+    if (famsa_rows_pairs(i0, i1) == 0) return FAMSA_OK;
+    FAMSA_CUDA(cudaSetDevice(ctx->device));
+    return sweep_rows(ctx, i0, i1, lcs_out, sim_out, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_host, float* sim_host) {
+    if (!ctx) { set_error("famsa_lcs_rows_host: ctx is NULL"); return FAMSA_EINVAL; }
+    if (i0 < 0 || i0 > i1 || i1 > ctx->k) { set_error("famsa_lcs_rows_host: bad row range"); return FAMSA_ERANGE; }
+    if (!lcs_host && !sim_host) { set_error("famsa_lcs_rows_host: both outputs are NULL"); return FAMSA_EINVAL; }
+    if (famsa_rows_pairs(i0, i1) == 0) return FAMSA_OK;
+    FAMSA_CUDA(cudaSetDevice(ctx->device));
+    // lazily create the ping-pong staging (two row-block buffers of up to 32 Mi pairs each)
+    const size_t want = (size_t)std::min<int64_t>(famsa_rows_pairs(i0, i1), (int64_t)32 << 20);
+    if (!ctx->s_compute) {
+        FAMSA_CUDA(cudaStreamCreateWithFlags(&ctx->s_compute, cudaStreamNonBlocking));
+        FAMSA_CUDA(cudaStreamCreateWithFlags(&ctx->s_copy, cudaStreamNonBlocking));
+        for (int b = 0; b < 2; ++b) {
+            FAMSA_CUDA(cudaEventCreateWithFlags(&ctx->ev_done[b], cudaEventDisableTiming));
+            FAMSA_CUDA(cudaEventCreateWithFlags(&ctx->ev_copied[b], cudaEventDisableTiming));
+        }
+    }
+    if (ctx->buf_pairs < want) {
+        FAMSA_CUDA(cudaDeviceSynchronize());
+        for (int b = 0; b < 2; ++b) {
+            cudaFree(ctx->d_lcs_buf[b]); cudaFree(ctx->d_sim_buf[b]);
+            ctx->d_lcs_buf[b] = nullptr; ctx->d_sim_buf[b] = nullptr;
+        }
+        ctx->buf_pairs = 0;
+        for (int b = 0; b < 2; ++b) {
+            cudaError_t e1 = cudaMalloc((void**)&ctx->d_lcs_buf[b], want * sizeof(uint16_t));
+            cudaError_t e2 = cudaMalloc((void**)&ctx->d_sim_buf[b], want * sizeof(float));
+            if (e1 != cudaSuccess || e2 != cudaSuccess) {
+                cudaGetLastError(); set_error("famsa_lcs_rows_host: device allocation failed"); return FAMSA_ENOMEM;
+            }
+        }
+        ctx->buf_pairs = want;
+    }
+    // chunk the row range so that each chunk fits a buffer (a single row always fits: i < 2^32 / ... k <= buf)
+    int64_t r = i0; int n = 0; int64_t done_pairs = 0;
+    while (r < i1) {
+        int64_t e = r + 1;
+        while (e < i1 && famsa_rows_pairs(r, e + 1) <= (int64_t)ctx->buf_pairs) ++e;
+        const int64_t np = famsa_rows_pairs(r, e);
+        if (np > (int64_t)ctx->buf_pairs) { set_error("famsa_lcs_rows_host: a single row exceeds the staging buffer"); return FAMSA_ENOMEM; }
+        const int b = n & 1;
+        if (n >= 2) FAMSA_CUDA(cudaStreamWaitEvent(ctx->s_compute, ctx->ev_copied[b], 0));
+        int rc = sweep_rows(ctx, r, e, lcs_host ? ctx->d_lcs_buf[b] : nullptr, sim_host ? ctx->d_sim_buf[b] : nullptr, ctx->s_compute);
+        if (rc != FAMSA_OK) return rc;
+        FAMSA_CUDA(cudaEventRecord(ctx->ev_done[b], ctx->s_compute));
+        FAMSA_CUDA(cudaStreamWaitEvent(ctx->s_copy, ctx->ev_done[b], 0));
+        if (lcs_host) FAMSA_CUDA(cudaMemcpyAsync(lcs_host + done_pairs, ctx->d_lcs_buf[b], np * sizeof(uint16_t), cudaMemcpyDeviceToHost, ctx->s_copy));
+        if (sim_host) FAMSA_CUDA(cudaMemcpyAsync(sim_host + done_pairs, ctx->d_sim_buf[b], np * sizeof(float), cudaMemcpyDeviceToHost, ctx->s_copy));
+        FAMSA_CUDA(cudaEventRecord(ctx->ev_copied[b], ctx->s_copy));
+        done_pairs += np; r = e; ++n;
+    }
+    FAMSA_CUDA(cudaStreamSynchronize(ctx->s_copy));
+    FAMSA_CUDA(cudaStreamSynchronize(ctx->s_compute));
+    return FAMSA_OK;
+}
