@@ -1,0 +1,366 @@
+#!/usr/bin/env python
+"""bench.py -- all-pairs LCS GCUPS / pairs/s on B200 and the fraction of the integer-ALU roofline
+(BASELINE.json `metric`), on the seeded synthetic stand-in for the paper's k = 415 519 family
+(BASELINE.json configs[4], the workload the north_star target is stated on).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--stride S] [--full]
+    python bench.py --impl reference ...      # the CPU oracle, as it stands, on the host cores
+
+A "step" is one pass of the whole sweep path (pair sweep -> zero count -> similarity epilogue ->
+row-block store) over one batch of row blocks of the packed set, inputs
+resident in HBM.  For configs 0-2 the batch is ALL rows (the full all-pairs job); for configs 3-4
+it is every `stride`-th 1024-row block (default 16), because a full sweep of config 4 takes most
+of a minute -- the rate counts true |A|*|B| cells only, so the subset changes the duration, not
+the metric; one full sweep is timed as well (`full_sweep`) unless --no-full.  famsa_pack (a1-a3,
+one-off) is timed separately (`pack_ms`) and is inside every e2e step.
+Prints ONE JSON line (rank 0).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "all_pairs_lcs_gcups"
+UNIT = "GCUPS"
+BLOCK_ROWS = 1024
+ALU_INSTR_PER_CELL = 3.0 / 32.0      # LOP3 + IADD3.X + LOP3 per 32-bit word-step
+WORKLOADS = {
+    0: "configs[0]: k=500, one family, all 124750 pairs",
+    1: "configs[1]: k=10000, 20 families, full all-pairs in 1024-row blocks",
+    2: "configs[2]: k=50000 length-skewed set (10% 1500-4000 residues), all pairs",
+    3: "configs[3]: k=100000 single family + 2% fragments, uint16 LCS only",
+    4: "configs[4]: k=415519 single family, lognormal lengths (mean ~300)",
+}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--k", type=int, default=None, help="override member count (debugging)")
+    ap.add_argument("--stride", type=int, default=None, help="row-block stride of a step (default: 1 for configs 0-2, 16 for 3-4)")
+    ap.add_argument("--full", action="store_true", help="a step is the full sweep whatever the config")
+    ap.add_argument("--no-full", action="store_true", help="skip the extra single full sweep")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU work per oracle sample")
+    return ap.parse_args()
+
+
+def step_blocks(k, stride, offset=0):
+    """Row blocks [i0, i1) of one step: every `stride`-th 1024-row block starting at `offset`."""
+    nblocks = (k + BLOCK_ROWS - 1) // BLOCK_ROWS
+    return [(b * BLOCK_ROWS, min((b + 1) * BLOCK_ROWS, k)) for b in range(offset % max(stride, 1), nblocks, stride)]
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device):
+        self.device = device
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.device), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [l.strip().split(", ") for l in open(self.f.name) if l.strip()]
+        os.unlink(self.f.name)
+        sm, reasons = [], set()
+        for r in rows:
+            if len(r) < 9:
+                continue
+            try:
+                sm.append(float(r[1])); out["sm_max_mhz"] = float(r[2])
+            except ValueError:
+                continue
+            for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], r[5:9]):
+                if v.strip().lower() == "active":
+                    reasons.add(name)
+        if sm:
+            out["sm_mhz"] = float(np.median(sm)); out["samples"] = len(sm)
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def oracle_sample(seqs, offsets, blocks, cpu_seconds, seed):
+    """A bounded seeded sample of the step's pairs for the CPU oracle: uniform over the pairs of
+    the step's row blocks, cut where the cell count reaches ~cpu_seconds of work on all cores
+    (planning rate 0.3 GCUPS per core).  Returns (orig_i, orig_j, cells, cores)."""
+    from oracle import famsa_oracle
+    cores = famsa_oracle.n_threads_default()
+    perm = famsa_oracle.sort_perm(offsets)
+    lens = np.diff(offsets)[perm].astype(np.int64)
+    rows = np.concatenate([np.arange(max(a, 1), b, dtype=np.int64) for a, b in blocks]) if blocks else np.zeros(0, np.int64)
+    if rows.size == 0:
+        z = np.zeros(0, np.int64)
+        return z, z, 0.0, cores
+    rng = np.random.default_rng(seed)
+    n = 400000
+    i = rng.choice(rows, size=n, p=rows / rows.sum())
+    j = (rng.random(n) * i).astype(np.int64)
+    cells = lens[i] * lens[j]
+    budget = 0.3e9 * cores * cpu_seconds
+    cut = int(np.searchsorted(np.cumsum(cells), budget)) + 1
+    cut = min(cut, n)
+    return perm[i[:cut]], perm[j[:cut]], float(cells[:cut].sum()), cores
+
+
+def time_oracle(seqs, offsets, pi, pj, want_sim):
+    from oracle import famsa_oracle
+    t0 = time.perf_counter()
+    famsa_oracle.pairs(seqs, offsets, pi, pj, want_sim=want_sim)
+    return time.perf_counter() - t0
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle as it stands, on the host cores; rank 0 only."""
+    if rank != 0:
+        return
+    from paper_1603_06958_b200 import synth
+    seqs, offsets = synth.family(args.config, k=args.k)
+    k = len(offsets) - 1
+    stride = args.stride or (1 if args.config <= 2 else 16)
+    blocks = step_blocks(k, 1 if args.full else stride)
+    want_sim = args.config != 3
+    secs = min(args.cpu_seconds, 8.0)
+    times, cells_step, pairs_step, cores = [], 0.0, 0, 1
+    for s in range(args.warmup + args.steps):
+        pi, pj, cells, cores = oracle_sample(seqs, offsets, blocks, secs, seed=1000 + s)
+        dt = time_oracle(seqs, offsets, pi, pj, want_sim)
+        if s >= args.warmup:
+            times.append(dt); cells_step += cells; pairs_step += pi.size
+    total = sum(times)
+    value = cells_step / total / 1e9
+    sample = "%d seeded uniform pairs of the step's row blocks per step (~%.0f s of CPU work)" % (pairs_step // max(args.steps, 1), secs)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": total / max(args.steps, 1) * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.config], "k": k, "step": "bounded oracle sample of the cuda arm's step"},
+        "pairs_per_s": pairs_step / total,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_cuda(args, rank, world, local_rank):
+    import torch
+    from paper_1603_06958_b200 import famsa as F, synth
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+
+    seqs, offsets = synth.family(args.config, k=args.k)      # replicated on every rank
+    k = len(offsets) - 1
+    want_sim = args.config != 3                               # configs[3]: uint16 row blocks only
+    stride = 1 if args.full else (args.stride or (1 if args.config <= 2 else 16))
+    # weak scaling: rank r sweeps its own batch of row blocks (offset r), same size as the N=1 batch
+    blocks = step_blocks(k, stride, offset=rank if stride > 1 else 0)
+    # (stride 1: the batch is the whole job, so every rank sweeps its own replica of it)
+
+    peak0 = F.famsa_alu_peak(local_rank)
+    t0 = time.perf_counter()
+    ctx = F.famsa_pack(seqs, offsets, device=local_rank)
+    torch.cuda.synchronize()
+    pack_ms = (time.perf_counter() - t0) * 1e3
+    pack_launches = F.famsa_launch_count(ctx)
+
+    max_pairs = max(F.famsa_rows_pairs(a, b) for a, b in blocks)
+    bufs = [(torch.empty(max_pairs, dtype=torch.uint16, device=dev),
+             torch.empty(max_pairs, dtype=torch.float32, device=dev) if want_sim else None) for _ in range(2)]
+    cells_step = sum(F.famsa_rows_cells(ctx, a, b) for a, b in blocks)
+    pairs_step = sum(F.famsa_rows_pairs(a, b) for a, b in blocks)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        for n, (a, b) in enumerate(blocks):
+            lcs, sim = bufs[n & 1]                            # ping-pong: the consumer owns one block while the next is swept
+            F.famsa_lcs_rows(ctx, a, b, lcs, sim, stream)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    l0 = F.famsa_launch_count(ctx)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    ev[0].record(stream)
+    for s in range(args.steps):
+        step()
+        ev[s + 1].record(stream)
+    barrier()
+    clocks = sampler.stop()
+    launches = F.famsa_launch_count(ctx) - l0
+    ms_total = ev[0].elapsed_time(ev[-1])
+    step_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)]
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+        tot = torch.tensor([cells_step, float(pairs_step)], dtype=torch.float64, device=dev)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        cells_all, pairs_all = float(tot[0].item()), float(tot[1].item())
+    else:
+        cells_all, pairs_all = cells_step, float(pairs_step)
+    sec = ms_total * 1e-3
+    value = cells_all * args.steps / sec / 1e9
+
+    # ---- e2e: HOST buffers through the C ABI; pack (H2D of the residues) + sweep + D2H every step
+    h_lcs = torch.empty(max_pairs, dtype=torch.uint16).pin_memory()
+    h_sim = torch.empty(max_pairs, dtype=torch.float32).pin_memory() if want_sim else None
+    e2e_steps = max(1, min(args.steps, 2))
+    def e2e_step():
+        c2 = F.famsa_pack(seqs, offsets, device=local_rank)
+        for a, b in blocks:
+            F.famsa_lcs_rows_host(c2, a, b, h_lcs, h_sim)
+        c2.free()
+    e2e_step()                                                # warm-up (allocations, staging buffers)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    barrier()
+    e2e_sec = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_sec], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_sec = float(t.item())
+    e2e_value = cells_all * e2e_steps / e2e_sec / 1e9
+    h2d = int(seqs.nbytes + offsets.nbytes)
+    d2h = int(pairs_step * (2 + (4 if want_sim else 0)))
+
+    # ---- one full sweep, timed alone (N = 1, configs 3-4 only: the other configs' step already is one)
+    full = None
+    if stride > 1 and world == 1 and not args.no_full:
+        allb = step_blocks(k, 1)
+        big = max(F.famsa_rows_pairs(a, b) for a, b in allb)
+        if big > max_pairs:
+            bufs = None
+            torch.cuda.empty_cache()
+            bufs = [(torch.empty(big, dtype=torch.uint16, device=dev),
+                     torch.empty(big, dtype=torch.float32, device=dev) if want_sim else None) for _ in range(2)]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for n, (a, b) in enumerate(allb):
+            F.famsa_lcs_rows(ctx, a, b, bufs[n & 1][0], bufs[n & 1][1], stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        fms = e0.elapsed_time(e1)
+        fcells = F.famsa_rows_cells(ctx, 0, k)
+        full = {"ms": fms, "gcups": fcells / fms / 1e6, "pairs": F.famsa_rows_pairs(0, k),
+                "pairs_per_s": F.famsa_rows_pairs(0, k) / fms * 1e3, "cells": fcells}
+    peak1 = F.famsa_alu_peak(local_rank)
+    ctx.free()
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- rank 0: the oracle beside it, the roofline, the line
+    cpu = None
+    if not args.no_cpu:
+        pi, pj, ccells, cores = oracle_sample(seqs, offsets, blocks, args.cpu_seconds, seed=7)
+        dt = time_oracle(seqs, offsets, pi, pj, want_sim)
+        cpu = {"value": ccells / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "pairs_per_s": pi.size / dt,
+               "sample": "%d seeded uniform pairs of the step's row blocks (%.3g cells, %.1f s)" % (pi.size, ccells, dt)}
+    p_int = max(peak0["instr_per_s"], peak1["instr_per_s"])          # measured INT32 ALU-pipe rate (thread-instr/s)
+    sm_count = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    achieved = cells_step * args.steps * ALU_INSTR_PER_CELL / (ev[0].elapsed_time(ev[-1]) * 1e-3)   # this rank's stream
+    peaks_file = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    sm_max = 1965.0
+    if os.path.exists(peaks_file):
+        sm_max = float(json.load(open(peaks_file)).get("sm_max_mhz", sm_max))
+    nominal = sm_count * 64 * sm_max * 1e6
+    roofline = {
+        "bound": "alu", "achieved": achieved / 1e12, "peak": p_int / 1e12, "unit": "TIOP/s (int32 ALU-pipe lane-instr)",
+        "frac": achieved / p_int, "traffic": None,
+        "kernel": "famsa::sweep_short_kernel<W> (%d launches per step)" % (launches // max(args.steps, 1)),
+        "algorithmic_instr_per_cell": ALU_INSTR_PER_CELL,
+        "peak_source": "famsa_alu_peak micro-kernel, measured in this run (MEASURED_PEAKS.json has no integer peak)",
+        "peak_instr_per_clk_sm": max(peak0["instr_per_clk_sm"], peak1["instr_per_clk_sm"]),
+        "peak_sm_mhz": max(peak0["sm_mhz"], peak1["sm_mhz"]),
+        "frac_of_nominal_64_per_clk_sm_at_max_clock": achieved / nominal,
+        "roofline_gcups": p_int / ALU_INSTR_PER_CELL / 1e9,
+    }
+    out_bytes = pairs_step * (2 + (4 if want_sim else 0))
+    if out_bytes > 126e6:
+        l2_note = "no flush needed: every step writes %.2f GB of row-block output (> 126 MB L2) between re-reads" % (out_bytes / 1e9)
+    else:
+        l2_note = "working set fits L2 (small config); ALU-bound path, no L2 flush between steps"
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32", "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.config], "k": k,
+                   "step": ("all rows" if stride == 1 else "every %d-th %d-row block (%d blocks)" % (stride, BLOCK_ROWS, len(blocks))),
+                   "pairs_per_step": pairs_step, "cells_per_step": cells_step, "outputs": "uint16 LCS" + (" + fp32 similarity" if want_sim else ""),
+                   "l2": l2_note,
+                   "parallelism": "replicated set, row blocks dealt per rank, no collective"},
+        "pairs_per_s": pairs_all * args.steps / sec,
+        "step_ms": step_ms, "pack_ms": pack_ms,
+        "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"], "samples": clocks["samples"]},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+                "what": "famsa_pack from host memory + famsa_lcs_rows_host into a pinned host row-block buffer, every step"},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+        "output_gb_per_s": pairs_all * args.steps * (2 + (4 if want_sim else 0)) / sec / 1e9,
+    }
+    if full is not None:
+        line["full_sweep"] = full
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    run_cuda(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

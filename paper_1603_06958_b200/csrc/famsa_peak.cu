@@ -1,7 +1,8 @@
 // famsa_peak.cu -- measures the roofline denominator: the chip's INT32 ALU-pipe issue rate.
 // MEASURED_PEAKS.json carries no integer peak, so the library measures one:
-// 8 independent chains per thread, each a LOP3 -> IADD3 -> LOP3 triple (the same instruction mix
-// as one word-step of the sweep, without the shared-memory load), all SMs, full occupancy.
+// 8 word-steps per thread and step, each LOP3 -> IADD3.X -> LOP3 (+ one LOP3 that keeps the mask
+// live), the adds linked by the hardware carry exactly as in the sweep so that ptxas cannot move
+// them to the FMA pipe as IMAD.IADD; no shared-memory load; all SMs, 32 warps per SM.
 #include "famsa_internal.h"
 
 namespace famsa {
@@ -17,6 +18,7 @@ __global__ void __launch_bounds__(256) alu_peak_kernel(uint32_t* out, uint32_t s
         v[c] = seed ^ (threadIdx.x * 2654435761u + c * 40503u);
         m[c] = (seed >> 3) + blockIdx.x * 97u + c;
     }
+    { uint32_t z = 0; asm volatile("add.cc.u32 %0, %0, %0;" : "+r"(z)); }      // define the carry flag
     long long t0 = clock64();
 #pragma unroll 1
     for (int it = 0; it < PEAK_ITERS; ++it) {
@@ -25,7 +27,8 @@ __global__ void __launch_bounds__(256) alu_peak_kernel(uint32_t* out, uint32_t s
 #pragma unroll
             for (int c = 0; c < PEAK_CHAINS; ++c) {
                 uint32_t x = v[c] & m[c];                 // LOP3
-                uint32_t s = v[c] + x;                    // IADD3
+                uint32_t s;                               // IADD3 / IADD3.X: the carry keeps it on the ALU pipe
+                asm volatile("addc.cc.u32 %0, %1, %2;" : "=r"(s) : "r"(v[c]), "r"(x));   // carry never dies
                 v[c] = s | (v[c] & ~m[(c + 1) % PEAK_CHAINS]);   // LOP3
                 m[c] ^= s;                                // keeps m live and loop-variant (LOP3)
             }

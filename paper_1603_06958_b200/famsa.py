@@ -1,0 +1,210 @@
+"""Thin binding over libfamsa_lcs.so (include/famsa_lcs.h): argument marshalling only.
+
+Same names as the C ABI.  Every step of the path runs in the library's CUDA kernels; torch
+supplies device memory and streams.  There is NO CPU fallback: if the library is missing or
+no sm_100 device is present, the calls raise.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfamsa_lcs.so")
+
+FAMSA_OK, FAMSA_EINVAL, FAMSA_ESYMBOL, FAMSA_ELENGTH, FAMSA_ERANGE, FAMSA_ENOMEM, FAMSA_ECUDA = 0, -1, -2, -3, -4, -5, -6
+FAMSA_MAX_LEN = 65535
+
+EXPORTS = ["famsa_pack", "famsa_lcs_rows", "famsa_lcs_rows_host", "famsa_rows_pairs", "famsa_rows_cells",
+           "famsa_k", "famsa_perm", "famsa_lengths", "famsa_codes", "famsa_match", "famsa_launch_count",
+           "famsa_alu_peak", "famsa_set_tuning", "famsa_free", "famsa_strerror", "famsa_last_error"]
+
+
+class FamsaError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("famsa error %d: %s" % (code, text))
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """The loaded C-ABI library.  Raises (never falls back) if it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libfamsa_lcs.so is not built (run `python -m paper_1603_06958_b200.build`); "
+                              "there is no CPU fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+        L.famsa_pack.restype = i32
+        L.famsa_pack.argtypes = [vp, vp, i64, i32, ctypes.POINTER(vp)]
+        L.famsa_lcs_rows.restype = i32
+        L.famsa_lcs_rows.argtypes = [vp, i64, i64, vp, vp, vp]
+        L.famsa_lcs_rows_host.restype = i32
+        L.famsa_lcs_rows_host.argtypes = [vp, i64, i64, vp, vp]
+        L.famsa_rows_pairs.restype = i64
+        L.famsa_rows_pairs.argtypes = [i64, i64]
+        L.famsa_rows_cells.restype = i32
+        L.famsa_rows_cells.argtypes = [vp, i64, i64, ctypes.POINTER(ctypes.c_double)]
+        L.famsa_k.restype = i32
+        L.famsa_k.argtypes = [vp, ctypes.POINTER(i64)]
+        L.famsa_perm.restype = i32
+        L.famsa_perm.argtypes = [vp, vp]
+        L.famsa_lengths.restype = i32
+        L.famsa_lengths.argtypes = [vp, vp]
+        L.famsa_codes.restype = i32
+        L.famsa_codes.argtypes = [vp, i64, vp]
+        L.famsa_match.restype = i32
+        L.famsa_match.argtypes = [vp, i64, i32, vp]
+        L.famsa_launch_count.restype = i64
+        L.famsa_launch_count.argtypes = [vp]
+        L.famsa_alu_peak.restype = i32
+        L.famsa_alu_peak.argtypes = [i32] + [ctypes.POINTER(ctypes.c_double)] * 3
+        L.famsa_set_tuning.restype = i32
+        L.famsa_set_tuning.argtypes = [i32]
+        L.famsa_free.restype = None
+        L.famsa_free.argtypes = [vp]
+        L.famsa_strerror.restype = ctypes.c_char_p
+        L.famsa_strerror.argtypes = [i32]
+        L.famsa_last_error.restype = ctypes.c_char_p
+        L.famsa_last_error.argtypes = []
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != FAMSA_OK:
+        L = lib()
+        detail = L.famsa_last_error().decode() or L.famsa_strerror(rc).decode()
+        raise FamsaError(rc, detail)
+
+
+def _ptr(t):
+    """Raw pointer of a torch tensor / numpy array / None."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        return t.ctypes.data
+    return t.data_ptr()
+
+
+class Ctx:
+    """Owns a famsa_ctx*.  Use as a context manager or call free()."""
+
+    def __init__(self, handle):
+        self.handle = handle
+
+    def free(self):
+        if self.handle:
+            lib().famsa_free(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.free()
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+def famsa_pack(seqs, offsets, device=0):
+    """seqs: uint8 numpy array / bytes (HOST); offsets: int64[k+1] (HOST).  Returns Ctx."""
+    if isinstance(seqs, (bytes, bytearray, str)):
+        seqs = np.frombuffer(seqs.encode("ascii") if isinstance(seqs, str) else bytes(seqs), dtype=np.uint8)
+    seqs = np.ascontiguousarray(seqs, dtype=np.uint8)
+    offsets = np.ascontiguousarray(offsets, dtype=np.int64)
+    k = offsets.size - 1
+    out = ctypes.c_void_p()
+    _check(lib().famsa_pack(seqs.ctypes.data if seqs.size else None, offsets.ctypes.data, k, int(device),
+                            ctypes.byref(out)))
+    return Ctx(out.value)
+
+
+def famsa_rows_pairs(i0, i1):
+    return int(lib().famsa_rows_pairs(int(i0), int(i1)))
+
+
+def famsa_lcs_rows(ctx, i0, i1, lcs_out, sim_out, cuda_stream=None):
+    """lcs_out: torch.uint16/int16 CUDA tensor or None; sim_out: torch.float32 CUDA tensor or None
+    (each with >= famsa_rows_pairs(i0, i1) elements).  Work is enqueued on cuda_stream (an int
+    cudaStream_t, a torch.cuda.Stream, or None = torch's current stream)."""
+    if cuda_stream is None:
+        import torch
+        cuda_stream = torch.cuda.current_stream().cuda_stream
+    elif hasattr(cuda_stream, "cuda_stream"):
+        cuda_stream = cuda_stream.cuda_stream
+    n = famsa_rows_pairs(i0, i1)
+    for t, size in ((lcs_out, 2), (sim_out, 4)):
+        if t is not None:
+            assert t.is_cuda and t.is_contiguous() and t.element_size() == size and t.numel() >= n
+    _check(lib().famsa_lcs_rows(ctx.handle, int(i0), int(i1), _ptr(lcs_out), _ptr(sim_out), cuda_stream))
+
+
+def famsa_lcs_rows_host(ctx, i0, i1, lcs_host, sim_host):
+    """HOST outputs: numpy arrays or CPU torch tensors (pinned or pageable), or None."""
+    n = famsa_rows_pairs(i0, i1)
+    for t, size in ((lcs_host, 2), (sim_host, 4)):
+        if t is not None:
+            if isinstance(t, np.ndarray):
+                assert t.flags.c_contiguous and t.itemsize == size and t.size >= n
+            else:
+                assert (not t.is_cuda) and t.is_contiguous() and t.element_size() == size and t.numel() >= n
+    _check(lib().famsa_lcs_rows_host(ctx.handle, int(i0), int(i1), _ptr(lcs_host), _ptr(sim_host)))
+
+
+def famsa_rows_cells(ctx, i0, i1):
+    c = ctypes.c_double()
+    _check(lib().famsa_rows_cells(ctx.handle, int(i0), int(i1), ctypes.byref(c)))
+    return c.value
+
+
+def famsa_k(ctx):
+    k = ctypes.c_int64()
+    _check(lib().famsa_k(ctx.handle, ctypes.byref(k)))
+    return k.value
+
+
+def famsa_perm(ctx):
+    out = np.empty(famsa_k(ctx), dtype=np.int64)
+    _check(lib().famsa_perm(ctx.handle, out.ctypes.data))
+    return out
+
+
+def famsa_lengths(ctx):
+    out = np.empty(famsa_k(ctx), dtype=np.uint32)
+    _check(lib().famsa_lengths(ctx.handle, out.ctypes.data))
+    return out
+
+
+def famsa_codes(ctx, s, length):
+    out = np.empty(int(length), dtype=np.uint8)
+    _check(lib().famsa_codes(ctx.handle, int(s), out.ctypes.data))
+    return out
+
+
+def famsa_match(ctx, s, c, length):
+    out = np.empty((int(length) + 31) // 32, dtype=np.uint32)
+    _check(lib().famsa_match(ctx.handle, int(s), int(c), out.ctypes.data))
+    return out
+
+
+def famsa_launch_count(ctx):
+    return int(lib().famsa_launch_count(ctx.handle))
+
+
+def famsa_alu_peak(device=0):
+    """Returns dict(instr_per_s, instr_per_clk_sm, sm_mhz): the measured INT32 ALU-pipe rate."""
+    a, b, c = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    _check(lib().famsa_alu_peak(int(device), ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
+    return {"instr_per_s": a.value, "instr_per_clk_sm": b.value, "sm_mhz": c.value}
+
+
+def famsa_set_tuning(rows_per_cta):
+    _check(lib().famsa_set_tuning(int(rows_per_cta)))

@@ -1,0 +1,230 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Bar: uint16 LCS bit-exact; fp32 similarity within 1e-6 relative of the
+oracle's float64 (inf == inf) -- BASELINE.json north_star."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+SIM_RTOL = 1e-6
+LETTERS = "ACDEFGHIKLMNPQRSTVWYBZXUO"
+
+
+@pytest.fixture(scope="module")
+def F():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1603_06958_b200 import build, famsa
+    build.build()
+    famsa.lib()              # raises if the extension is missing: no fallback
+    return famsa
+
+
+def gpu_rows(F, ctx, i0, i1, want_lcs=True, want_sim=True):
+    import torch
+    n = F.famsa_rows_pairs(i0, i1)
+    lcs = torch.full((max(n, 1),), 0xFFFF, dtype=torch.uint16, device="cuda") if want_lcs else None
+    sim = torch.full((max(n, 1),), -1.0, dtype=torch.float32, device="cuda") if want_sim else None
+    F.famsa_lcs_rows(ctx, i0, i1, lcs, sim)
+    torch.cuda.synchronize()
+    return (lcs.cpu().numpy()[:n].astype(np.int64) if want_lcs else None,
+            sim.cpu().numpy()[:n] if want_sim else None)
+
+
+def assert_match(lcs_gpu, sim_gpu, lcs_ref, sim_ref):
+    if lcs_gpu is not None:
+        bad = np.flatnonzero(lcs_gpu != lcs_ref)
+        assert bad.size == 0, "LCS mismatch at %s: gpu %s oracle %s" % (bad[:5], lcs_gpu[bad[:5]], lcs_ref[bad[:5]])
+    if sim_gpu is not None:
+        inf_ref = np.isinf(sim_ref)
+        assert np.array_equal(np.isinf(sim_gpu) & (sim_gpu > 0), inf_ref)
+        fin = ~inf_ref
+        err = np.abs(sim_gpu[fin].astype(np.float64) - sim_ref[fin])
+        assert np.all(err <= SIM_RTOL * np.abs(sim_ref[fin])), float((err / np.maximum(np.abs(sim_ref[fin]), 1e-300)).max())
+
+
+def check_all_rows(F, oracle, seqs, offsets, i0=0, i1=None):
+    k = len(offsets) - 1
+    i1 = k if i1 is None else i1
+    with F.famsa_pack(seqs, offsets) as ctx:
+        lcs, sim = gpu_rows(F, ctx, i0, i1)
+    lref, sref = oracle.rows(seqs, offsets, i0, i1)
+    assert_match(lcs, sim, lref, sref)
+    return lcs, sim
+
+
+def make_set(seq_list):
+    arrs = [np.frombuffer(s.encode(), np.uint8) if isinstance(s, str) else np.asarray(s, np.uint8) for s in seq_list]
+    offsets = np.concatenate([[0], np.cumsum([a.size for a in arrs])]).astype(np.int64)
+    return (np.concatenate(arrs) if arrs else np.zeros(0, np.uint8)), offsets
+
+
+# ---- a1-a3: what pack builds ----------------------------------------------------------------
+def test_pack_roundtrip(F, oracle):
+    from paper_1603_06958_b200 import synth
+    seqs, offsets = synth.family(2, k=200, seed=5)          # short + long sequences (blocked tables)
+    with F.famsa_pack(seqs, offsets) as ctx:
+        assert F.famsa_k(ctx) == 200
+        perm = F.famsa_perm(ctx)
+        lens = F.famsa_lengths(ctx)
+        assert np.array_equal(perm, oracle.sort_perm(offsets))           # descending, stable (R15)
+        assert np.array_equal(lens, np.diff(offsets)[perm])
+        cells = F.famsa_rows_cells(ctx, 0, 200)
+        L = lens.astype(np.float64)
+        assert cells == pytest.approx(sum(L[i] * L[:i].sum() for i in range(200)), rel=1e-12)
+        for s in [0, 1, 19, 20, 31, 32, 100, 199]:
+            ref = oracle.encode(seqs[offsets[perm[s]]:offsets[perm[s] + 1]])
+            assert np.array_equal(F.famsa_codes(ctx, s, lens[s]), ref)
+            for c in [0, 9, 24, 25, 31]:
+                bits = np.zeros(((lens[s] + 31) // 32) * 32, np.uint8)
+                bits[:lens[s]] = ref == c                                # bit i of M[c] = (S[i] == c)
+                words = np.packbits(bits.reshape(-1, 32), axis=1, bitorder="little").view(np.uint32).ravel()
+                assert np.array_equal(F.famsa_match(ctx, s, c, lens[s]), words), (s, c)
+
+
+def test_letters_and_bad_symbols(F, oracle):
+    seqs, offsets = make_set(["ACDEFGHIKLMNPQRSTVWY", "acdefghiklmnpqrstvwy", "BZXUOJ", "bzxuoj", "MKVLAAGIVGL"])
+    lcs, sim = check_all_rows(F, oracle, seqs, offsets)
+    assert 20 in lcs and np.isinf(sim).sum() == 2        # case folded: two identical pairs
+    for bad in ["ACD*F", "ACD-F", "ACD F", "ACD1F", "ACD@F", "ACD[F", "ACD{F"]:
+        s, o = make_set(["ACDEF", bad])
+        with pytest.raises(F.FamsaError) as e:
+            F.famsa_pack(s, o)
+        assert e.value.code == F.FAMSA_ESYMBOL and "position 8" in str(e.value)
+    s, o = make_set([np.array([0, 1, 25], np.uint8)])
+    with pytest.raises(F.FamsaError) as e:
+        F.famsa_pack(s, o)
+    assert e.value.code == F.FAMSA_ESYMBOL
+
+
+# ---- a4-a7: the sweep -------------------------------------------------------------------------
+def test_config0_all_pairs(F, oracle):
+    """BASELINE.json configs[0]: k = 500, all 124 750 pairs."""
+    from paper_1603_06958_b200 import synth
+    seqs, offsets = synth.family(0)
+    lcs, sim = check_all_rows(F, oracle, seqs, offsets)
+    assert lcs.size == 124750
+    assert np.isinf(sim).sum() >= 3                      # the planted duplicates (R12)
+
+
+def test_degenerate_sizes(F, oracle):
+    import torch
+    for seq_list in ([], ["ACD"], ["ACD", "AC"], ["A", "A"], ["A", "C"]):
+        seqs, offsets = make_set(seq_list)
+        check_all_rows(F, oracle, seqs, offsets)
+    seqs, offsets = make_set(["ACDEF", "ACD", "AC"])
+    with F.famsa_pack(seqs, offsets) as ctx:
+        buf = torch.zeros(8, dtype=torch.uint16, device="cuda")
+        F.famsa_lcs_rows(ctx, 1, 1, buf, None)           # empty range: legal, writes nothing
+        F.famsa_lcs_rows(ctx, 0, 1, buf, None)           # row 0 is empty
+        assert int(buf.cpu().numpy().astype(np.int64).sum()) == 0
+        for i0, i1 in [(2, 1), (0, 4), (-1, 2)]:
+            with pytest.raises(F.FamsaError) as e:
+                F.famsa_lcs_rows(ctx, i0, i1, buf, None)
+            assert e.value.code == F.FAMSA_ERANGE
+        with pytest.raises(F.FamsaError) as e:
+            F.famsa_lcs_rows(ctx, 0, 3, None, None)
+        assert e.value.code == F.FAMSA_EINVAL
+
+
+def test_word_boundaries(F, oracle):
+    """|A| = 0, 1, 31 mod 32 and every register-path word count 1..32, plus the first blocked sizes."""
+    rng = np.random.default_rng(31)
+    lens = [1, 2, 31, 32, 33, 63, 64, 65, 95, 96, 97, 127, 128, 129, 255, 256, 257, 511, 512, 513,
+            991, 992, 993, 1023, 1024, 1025, 1055, 1056, 1057, 2047, 2048, 2049] + list(range(40, 1030, 32))
+    seq_list = [rng.integers(0, 4, n).astype(np.uint8) for n in lens]     # 4 letters: LCS is long, carries are busy
+    seqs, offsets = make_set(seq_list)
+    check_all_rows(F, oracle, seqs, offsets)
+
+
+def test_closed_forms_on_gpu(F, oracle):
+    """Inputs whose answer is known in closed form, independent of the oracle."""
+    n = 700
+    seq_list = ["A" * 1500, "A" * 64, "AC" * n, "CA" * n, "D" * 33, "W" * 1024, "W" * 1025]
+    seqs, offsets = make_set(seq_list)
+    with F.famsa_pack(seqs, offsets) as ctx:
+        perm = F.famsa_perm(ctx)
+        lcs, _ = gpu_rows(F, ctx, 0, len(seq_list))
+    inv = np.argsort(perm)
+    def get(a, b):
+        i, j = max(inv[a], inv[b]), min(inv[a], inv[b])
+        return lcs[i * (i - 1) // 2 + j]
+    assert get(0, 1) == 64 and get(2, 3) == 2 * n - 1 and get(0, 4) == 0
+    assert get(5, 6) == 1024 and get(0, 2) == n and get(1, 3) == 64
+
+
+def test_row_block_independence(F, oracle):
+    """(i, j) does not depend on block boundaries, tile shape or co-launched pairs."""
+    from paper_1603_06958_b200 import synth
+    seqs, offsets = synth.family(1, k=1300, seed=77)
+    k = 1300
+    with F.famsa_pack(seqs, offsets) as ctx:
+        full_lcs, full_sim = gpu_rows(F, ctx, 0, k)
+        for block in (1, 7, 1024):
+            lo = 1100 if block == 1 else (900 if block == 7 else 0)
+            for i0 in range(lo, k, block):
+                i1 = min(i0 + block, k)
+                l, s = gpu_rows(F, ctx, i0, i1)
+                a, b = F.famsa_rows_pairs(0, i0), F.famsa_rows_pairs(0, i1)
+                assert np.array_equal(l, full_lcs[a:b]) and np.array_equal(s, full_sim[a:b])
+        for ta in (1, 3, 12):
+            F.famsa_set_tuning(ta)
+            l, s = gpu_rows(F, ctx, 0, k)
+            assert np.array_equal(l, full_lcs) and np.array_equal(s, full_sim)
+        F.famsa_set_tuning(8)
+        l, _ = gpu_rows(F, ctx, 100, 300, want_sim=False)       # LCS only (configs[3])
+        _, s = gpu_rows(F, ctx, 100, 300, want_lcs=False)       # similarity only
+        a, b = F.famsa_rows_pairs(0, 100), F.famsa_rows_pairs(0, 300)
+        assert np.array_equal(l, full_lcs[a:b]) and np.array_equal(s, full_sim[a:b])
+        hl = np.empty(F.famsa_rows_pairs(0, k), np.uint16)
+        hs = np.empty(F.famsa_rows_pairs(0, k), np.float32)
+        F.famsa_lcs_rows_host(ctx, 0, k, hl, hs)                # the HOST-buffer entry point
+        assert np.array_equal(hl.astype(np.int64), full_lcs) and np.array_equal(hs, full_sim)
+    sel = np.arange(0, full_lcs.size, 97)
+    lref, sref = oracle.rows(seqs, offsets, 0, k)
+    assert_match(full_lcs, full_sim, lref, sref)
+    assert sel.size > 0
+
+
+def test_config2_long_path(F, oracle):
+    """BASELINE.json configs[2] recipe at k = 320: 1 500-4 000-residue sequences (blocked carry path)."""
+    from paper_1603_06958_b200 import synth
+    seqs, offsets = synth.family(2, k=320, seed=91)
+    assert np.diff(offsets).max() > 1500
+    check_all_rows(F, oracle, seqs, offsets)
+
+
+def test_config3_fragments_lcs_only(F, oracle):
+    from paper_1603_06958_b200 import synth
+    seqs, offsets = synth.family(3, k=600, seed=93)
+    with F.famsa_pack(seqs, offsets) as ctx:
+        lcs, _ = gpu_rows(F, ctx, 0, 600, want_sim=False)
+    lref, _ = oracle.rows(seqs, offsets, 0, 600, want_sim=False)
+    assert_match(lcs, None, lref, None)
+
+
+def test_maximum_lengths(F, oracle):
+    """FAMSA_MAX_LEN = 65535 and the large carry-vector variant (|B| > 4096)."""
+    rng = np.random.default_rng(37)
+    lens = [65535, 30000, 6000, 4097, 4096, 1025, 300, 1]
+    seq_list = [rng.integers(0, 20, n).astype(np.uint8) for n in lens]
+    seq_list.append(seq_list[2].copy())                           # a long duplicate: LCS = 6000, +inf
+    seqs, offsets = make_set(seq_list)
+    lcs, sim = check_all_rows(F, oracle, seqs, offsets)
+    assert 6000 in lcs and np.isinf(sim).sum() == 1
+
+
+def test_planted_long(F):
+    """Planted common subsequence between disjoint-alphabet fillers: LCS known exactly, no oracle."""
+    rng = np.random.default_rng(41)
+    p = 1700
+    common = rng.integers(0, 8, p)
+    def embed(n, lo, hi):
+        out = rng.integers(lo, hi, n)
+        out[np.sort(rng.choice(n, p, replace=False))] = common
+        return out.astype(np.uint8)
+    seqs, offsets = make_set([embed(3900, 8, 16), embed(3500, 16, 24)])
+    with F.famsa_pack(seqs, offsets) as ctx:
+        lcs, sim = gpu_rows(F, ctx, 0, 2)
+    assert lcs[0] == p
+    assert sim[0] == pytest.approx(p / float(3900 + 3500 - 2 * p) ** 2, rel=1e-6)
