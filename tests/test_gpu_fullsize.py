@@ -1,0 +1,81 @@
+"""Full-size parity in the launch configuration bench.py times (1024-row blocks of the packed
+BASELINE.json configs[1] and configs[4] sets), on sampled outputs the oracle computes one by one."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+BLOCK_ROWS = 1024
+
+
+def check_blocks(F, oracle, seqs, offsets, block_ids, n_per_block, want_sim=True):
+    import torch
+    k = len(offsets) - 1
+    perm_ref = oracle.sort_perm(offsets)
+    checked = 0
+    with F.famsa_pack(seqs, offsets) as ctx:
+        assert np.array_equal(F.famsa_perm(ctx), perm_ref)
+        lens = F.famsa_lengths(ctx)
+        for b in block_ids:
+            i0, i1 = b * BLOCK_ROWS, min((b + 1) * BLOCK_ROWS, k)
+            n = F.famsa_rows_pairs(i0, i1)
+            lcs = torch.full((n,), 0xFFFF, dtype=torch.uint16, device="cuda")
+            sim = torch.full((n,), -1.0, dtype=torch.float32, device="cuda") if want_sim else None
+            F.famsa_lcs_rows(ctx, i0, i1, lcs, sim)
+            # seeded sample inside the block: uniform + first/last rows + word-boundary lengths
+            rng = np.random.default_rng(1000 + b)
+            lo = max(i0, 1)
+            rows = rng.integers(lo, i1, n_per_block)
+            rows[:64] = lo
+            rows[64:128] = i1 - 1
+            special = np.flatnonzero(np.isin(lens[lo:i1] % 32, (0, 1, 31))) + lo
+            if special.size:
+                rows[128:192] = rng.choice(special, 64)
+            cols = (rng.random(n_per_block) * rows).astype(np.int64)
+            cols[:8] = 0
+            cols[64:72] = rows[64:72] - 1                                  # first and last column of a row
+            pos = rows * (rows - 1) // 2 - i0 * (i0 - 1) // 2 + cols
+            idx = torch.from_numpy(pos).cuda()
+            torch.cuda.synchronize()
+            lg = lcs.view(torch.int16)[idx].cpu().numpy().view(np.uint16).astype(np.int64)
+            lref, sref = oracle.pairs(seqs, offsets, perm_ref[rows], perm_ref[cols], want_sim=want_sim)
+            assert np.array_equal(lg, lref), (b, np.flatnonzero(lg != lref)[:5])
+            if want_sim:
+                sg = sim[idx].cpu().numpy().astype(np.float64)
+                fin = np.isfinite(sref)
+                assert np.array_equal(np.isinf(sg), ~fin)
+                assert np.all(np.abs(sg[fin] - sref[fin]) <= 1e-6 * np.abs(sref[fin]))
+            # a property that holds for EVERY entry of the block, checked on the device:
+            # 0 < LCS <= |A| (row i is the shorter sequence) -- every entry was written
+            li = torch.from_numpy(np.repeat(lens[i0:i1].astype(np.int32), np.arange(i0, i1))).cuda()
+            lv = lcs.view(torch.int16).to(torch.int32).bitwise_and(0xFFFF)
+            assert bool((lv <= li).all())
+            del lcs, sim, li, lv
+            checked += n_per_block
+    return checked
+
+
+@pytest.fixture(scope="module")
+def F():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1603_06958_b200 import build, famsa
+    build.build()
+    return famsa
+
+
+def test_config1_full_size_sampled(F, oracle):
+    from paper_1603_06958_b200 import synth
+    seqs, offsets = synth.family(1)
+    assert len(offsets) - 1 == 10000
+    assert check_blocks(F, oracle, seqs, offsets, range(10), 2500) == 25000
+
+
+def test_config4_full_size_sampled(F, oracle):
+    """k = 415 519: the set bench.py times; blocks from the long end, the middle and the short end."""
+    from paper_1603_06958_b200 import synth
+    seqs, offsets = synth.family(4)
+    k = len(offsets) - 1
+    assert k == 415519
+    last = (k - 1) // BLOCK_ROWS
+    assert check_blocks(F, oracle, seqs, offsets, [0, 1, 96, 240, last - 1, last], 6000) == 36000
