@@ -172,6 +172,26 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def rank_blocks(k, stride, rank):
+    """The row blocks rank `rank` sweeps in one step.  Pairs are independent, so the path
+    shards with no data-path collective: the packed set is replicated and row blocks are dealt by rank.
+    stride > 1: rank r takes blocks r, r+stride, ... (disjoint batches of equal size: weak scaling);
+    stride 1: the batch is the whole job and every rank sweeps its own replica of it."""
+    return step_blocks(k, stride, offset=rank if stride > 1 else 0)
+
+
+def reduce_over_ranks(dist, ms, cells, pairs, device):
+    """Whole-job figures: MAX of the device time over ranks, SUM of the cells and pairs processed."""
+    if dist is None:
+        return ms, cells, float(pairs)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    tot = torch.tensor([cells, float(pairs)], dtype=torch.float64, device=device)
+    dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(tot[0].item()), float(tot[1].item())
+
+
 def run_cuda(args, rank, world, local_rank):
     import torch
     from paper_1603_06958_b200 import famsa as F, synth
@@ -187,8 +207,7 @@ def run_cuda(args, rank, world, local_rank):
     want_sim = args.config != 3                               # configs[3]: uint16 row blocks only
     stride = 1 if args.full else (args.stride or (1 if args.config <= 2 else 16))
     # weak scaling: rank r sweeps its own batch of row blocks (offset r), same size as the N=1 batch
-    blocks = step_blocks(k, stride, offset=rank if stride > 1 else 0)
-    # (stride 1: the batch is the whole job, so every rank sweeps its own replica of it)
+    blocks = rank_blocks(k, stride, rank)
 
     peak0 = F.famsa_alu_peak(local_rank)
     t0 = time.perf_counter()
@@ -230,15 +249,7 @@ def run_cuda(args, rank, world, local_rank):
     launches = F.famsa_launch_count(ctx) - l0
     ms_total = ev[0].elapsed_time(ev[-1])
     step_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)]
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-        tot = torch.tensor([cells_step, float(pairs_step)], dtype=torch.float64, device=dev)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-        cells_all, pairs_all = float(tot[0].item()), float(tot[1].item())
-    else:
-        cells_all, pairs_all = cells_step, float(pairs_step)
+    ms_total, cells_all, pairs_all = reduce_over_ranks(dist, ms_total, cells_step, pairs_step, dev)
     sec = ms_total * 1e-3
     value = cells_all * args.steps / sec / 1e9
 
