@@ -71,24 +71,33 @@ __device__ __forceinline__ void residue_step(uint32_t (&V)[W], uint32_t addr, ui
     for (int w = 0; w < W; ++w) V[w] = s[w] | (V[w] & ~m[w]);
 }
 
-template <int W, bool CARRY>
-__device__ __forceinline__ void word_step(uint32_t (&V)[W], uint32_t bword, uint32_t tbase, uint32_t& cin, uint32_t& cout) {
-    // byte r of bword is code*4 (< 128); tbase is 256-byte aligned, so PRMT splices the byte in.
-    residue_step<W, CARRY>(V, __byte_perm(bword, tbase, 0x7650), cin, cout);
-    residue_step<W, CARRY>(V, __byte_perm(bword, tbase, 0x7651), cin, cout);
-    residue_step<W, CARRY>(V, __byte_perm(bword, tbase, 0x7652), cin, cout);
-    residue_step<W, CARRY>(V, __byte_perm(bword, tbase, 0x7653), cin, cout);
+// Shared-memory address of residue R's symbol column: the table base with byte R of bword (= code*4
+// < 128) spliced into its low byte -- tbase is 256-byte aligned, so one PRMT does extract + add.
+// (Tried and rejected, r01: doing this on the FMA pipe with IMAD + IMAD.HI against __constant__
+// multipliers -- 7 FMA-pipe instructions per 4 residues instead of 4 ALU ones -- ran 3 % slower.)
+template <int R>
+__device__ __forceinline__ uint32_t residue_addr(uint32_t bword, uint32_t tbase) {
+    return __byte_perm(bword, tbase, 0x7650 + R);
 }
 
-// Sweep all chunks of this warp's group against one table block.  cv: carry bit-vector (16 bits
-// per chunk) or nullptr-equivalent when !CARRY.
 template <int W, bool CARRY>
-__device__ __forceinline__ void sweep_block(uint32_t (&V)[W], const uint4* __restrict__ bp, uint32_t nch, uint32_t tbase,
+__device__ __forceinline__ void word_step(uint32_t (&V)[W], uint32_t bword, uint32_t tbase, uint32_t& cin, uint32_t& cout) {
+    residue_step<W, CARRY>(V, residue_addr<0>(bword, tbase), cin, cout);
+    residue_step<W, CARRY>(V, residue_addr<1>(bword, tbase), cin, cout);
+    residue_step<W, CARRY>(V, residue_addr<2>(bword, tbase), cin, cout);
+    residue_step<W, CARRY>(V, residue_addr<3>(bword, tbase), cin, cout);
+}
+
+// Sweep this warp's group (nwords 4-residue words, i.e. up to the group's longest sequence) against
+// one table block.  cv: carry bit-vector, 16 bits per 16-residue chunk (blocked path only).
+template <int W, bool CARRY>
+__device__ __forceinline__ void sweep_block(uint32_t (&V)[W], const uint4* __restrict__ bp, uint32_t nwords, uint32_t tbase,
                                             unsigned short* cv, bool read_cv, bool write_cv) {
-    uint4 cur = nch ? __ldg(bp) : make_uint4(0, 0, 0, 0);
-    for (uint32_t c = 0; c < nch; ++c) {
+    const uint32_t nfull = nwords >> 2, tail = nwords & 3;
+    uint4 cur = nwords ? __ldg(bp) : make_uint4(0, 0, 0, 0);
+    for (uint32_t c = 0; c < nfull; ++c) {
         uint4 nxt = cur;
-        if (c + 1 < nch) nxt = __ldg(bp + (size_t)(c + 1) * GROUP);
+        if ((c + 1) * 4 < nwords) nxt = __ldg(bp + (size_t)(c + 1) * GROUP);
         uint32_t cin = 0, cout = 0;
         if (CARRY && read_cv) cin = (uint32_t)cv[c] << 16;
         word_step<W, CARRY>(V, cur.x, tbase, cin, cout);
@@ -97,6 +106,16 @@ __device__ __forceinline__ void sweep_block(uint32_t (&V)[W], const uint4* __res
         word_step<W, CARRY>(V, cur.w, tbase, cin, cout);
         if (CARRY && write_cv) cv[c] = (unsigned short)cout;
         cur = nxt;
+    }
+    if (tail) {                                           // last, partial chunk: 1-3 words
+        uint32_t cin = 0, cout = 0;
+        if (CARRY && read_cv) cin = (uint32_t)cv[nfull] << 16;
+#pragma unroll 1
+        for (uint32_t q = 0; q < tail; ++q) {
+            const uint32_t w = q == 0 ? cur.x : (q == 1 ? cur.y : cur.z);
+            word_step<W, CARRY>(V, w, tbase, cin, cout);
+        }
+        if (CARRY && write_cv) cv[nfull] = (unsigned short)(cout << (16 - 4 * tail));   // first residue's carry at bit 15
     }
 }
 
@@ -114,6 +133,7 @@ __device__ __forceinline__ void store_pair(const SweepArgs& a, uint32_t i, uint3
 template <int W>
 __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
     extern __shared__ __align__(256) uint8_t smem[];
+    asm volatile("griddepcontrol.launch_dependents;");
     constexpr int WST = (W + 1) & ~1;
     const uint32_t col_tile = blockIdx.x % a.n_col_tiles, row_tile = blockIdx.x / a.n_col_tiles;
     const uint32_t r_lo = a.r0 + row_tile * a.ta;
@@ -133,15 +153,16 @@ __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
     if (jw + 1 >= r_hi) return;                          // this warp's columns are all >= every row (no barrier follows)
     const uint32_t j = jw + lane;
     const uint32_t g = jw / GROUP;                       // jw < k, so g is a real group
-    const uint32_t gb = a.goff[g], nch = a.goff[g + 1] - gb;
+    const uint32_t gb = a.goff[g];
     const uint4* bp = a.stream + (size_t)gb * GROUP + lane;
     const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
     const uint32_t lb = j < r_hi ? a.len[j] : 0;         // columns >= r_hi are never stored
+    const uint32_t nwords = (a.len[jw] + 3) >> 2;        // 4-residue words to sweep: jw is the group's longest sequence
     for (uint32_t i = max(r_lo, jw + 1); i < r_hi; ++i) {
         uint32_t V[W];
 #pragma unroll
         for (int w = 0; w < W; ++w) V[w] = 0xFFFFFFFFu;
-        sweep_block<W, false>(V, bp, nch, smem_base + (i - r_lo) * (WST * ROW_BYTES), nullptr, false, false);
+        sweep_block<W, false>(V, bp, nwords, smem_base + (i - r_lo) * (WST * ROW_BYTES), nullptr, false, false);
         uint32_t lcs = 0;
 #pragma unroll
         for (int w = 0; w < W; ++w) lcs += __popc(~V[w]);
@@ -153,6 +174,7 @@ __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
 template <int W, int CW>
 __global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
     extern __shared__ __align__(256) uint8_t smem[];
+    asm volatile("griddepcontrol.launch_dependents;");
     constexpr int WST = (W + 1) & ~1;
     const uint32_t col_tile = blockIdx.x % a.n_col_tiles, row_tile = blockIdx.x / a.n_col_tiles;
     const uint32_t i = a.r0 + row_tile;
@@ -162,8 +184,8 @@ __global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
     const uint32_t jw = j0 + (threadIdx.x & ~31u);
     const uint32_t j = jw + lane;
     const bool active = jw < i;                          // warp-uniform
-    uint32_t gb = 0, nch = 0;
-    if (active) { const uint32_t g = jw / GROUP; gb = a.goff[g]; nch = a.goff[g + 1] - gb; }
+    const uint32_t gb = active ? a.goff[jw / GROUP] : 0;
+    const uint32_t nwords = active ? (a.len[jw] + 3) >> 2 : 0;
     const uint4* bp = a.stream + (size_t)gb * GROUP + lane;
     const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
     unsigned short cv[CW * 2];                           // 16 carry bits per 16-residue chunk
@@ -179,7 +201,7 @@ __global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
             uint32_t V[W];
 #pragma unroll
             for (int w = 0; w < W; ++w) V[w] = 0xFFFFFFFFu;
-            sweep_block<W, true>(V, bp, nch, smem_base, cv, blk > 0, blk + 1 < a.nblk);
+            sweep_block<W, true>(V, bp, nwords, smem_base, cv, blk > 0, blk + 1 < a.nblk);
 #pragma unroll
             for (int w = 0; w < W; ++w) lcs += __popc(~V[w]);
         }
@@ -192,19 +214,31 @@ __global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
 // ---- host side: buckets -> launches ------------------------------------------------------------
 namespace famsa {
 
+// Launches after the first one of a famsa_lcs_rows call carry the programmatic-stream-serialization
+// attribute: the launches of one call read the same read-only set and write disjoint output ranges,
+// so the next bucket's CTAs may fill the SMs while the previous launch drains its last wave
+// (every sweep kernel executes griddepcontrol.launch_dependents on entry; none needs .wait).
+template <typename K>
+static cudaError_t launch_sweep(K kernel, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st, bool overlap) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(TB); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = overlap ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, a);
+}
 template <int W>
-static cudaError_t launch_short(const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st) {
-    sweep_short_kernel<W><<<grid, TB, smem, st>>>(a);
-    return cudaGetLastError();
+static cudaError_t launch_short(const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st, bool overlap) {
+    return launch_sweep(sweep_short_kernel<W>, a, grid, smem, st, overlap);
 }
 template <int W, int CW>
-static cudaError_t launch_long(const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st) {
-    sweep_long_kernel<W, CW><<<grid, TB, smem, st>>>(a);
-    return cudaGetLastError();
+static cudaError_t launch_long(const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st, bool overlap) {
+    return launch_sweep(sweep_long_kernel<W, CW>, a, grid, smem, st, overlap);
 }
 
-#define SHORT_CASE(W) case W: return launch_short<W>(a, grid, smem, st);
-static cudaError_t dispatch_short(int w, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st) {
+#define SHORT_CASE(W) case W: return launch_short<W>(a, grid, smem, st, overlap);
+static cudaError_t dispatch_short(int w, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st, bool overlap) {
     switch (w) {
         SHORT_CASE(1) SHORT_CASE(2) SHORT_CASE(3) SHORT_CASE(4) SHORT_CASE(5) SHORT_CASE(6) SHORT_CASE(7) SHORT_CASE(8)
         SHORT_CASE(9) SHORT_CASE(10) SHORT_CASE(11) SHORT_CASE(12) SHORT_CASE(13) SHORT_CASE(14) SHORT_CASE(15) SHORT_CASE(16)
@@ -213,9 +247,9 @@ static cudaError_t dispatch_short(int w, const SweepArgs& a, unsigned grid, size
         default: return cudaErrorInvalidValue;
     }
 }
-#define LONG_CASE(W) case W: return launch_long<W, CW_SMALL>(a, grid, smem, st);
-static cudaError_t dispatch_long(int w, bool large, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st) {
-    if (large) return w == 32 ? launch_long<32, CW_LARGE>(a, grid, smem, st) : cudaErrorInvalidValue;
+#define LONG_CASE(W) case W: return launch_long<W, CW_SMALL>(a, grid, smem, st, overlap);
+static cudaError_t dispatch_long(int w, bool large, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st, bool overlap) {
+    if (large) return w == 32 ? launch_long<32, CW_LARGE>(a, grid, smem, st, overlap) : cudaErrorInvalidValue;
     switch (w) {
         LONG_CASE(17) LONG_CASE(18) LONG_CASE(19) LONG_CASE(20) LONG_CASE(21) LONG_CASE(22) LONG_CASE(23) LONG_CASE(24)
         LONG_CASE(25) LONG_CASE(26) LONG_CASE(27) LONG_CASE(28) LONG_CASE(29) LONG_CASE(30) LONG_CASE(31) LONG_CASE(32)
@@ -223,7 +257,7 @@ static cudaError_t dispatch_long(int w, bool large, const SweepArgs& a, unsigned
     }
 }
 
-static uint32_t g_rows_per_cta = 8;     // TA; tunable through famsa_set_tuning (tests sweep it)
+static uint32_t g_rows_per_cta = 2;     // TA; tunable through famsa_set_tuning (tests sweep it)
 
 int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim, cudaStream_t st) {
     SweepArgs a;
@@ -234,6 +268,7 @@ int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim
     a.len = ctx->d_len;
     a.lcs_out = lcs; a.sim_out = sim;
     a.out_base = i0 * (i0 - 1) / 2;
+    int n_launched = 0;
     for (const Bucket& b : ctx->buckets) {
         int64_t lo = std::max(b.r0, std::max<int64_t>(i0, 1)), hi = std::min(b.r1, i1);   // row 0 is empty
         for (int64_t r = lo; r < hi; r += MAX_ROWS_PER_LAUNCH) {
@@ -245,13 +280,13 @@ int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim
             if (b.nblk == 1) {
                 a.ta = g_rows_per_cta;
                 unsigned row_tiles = (a.r1 - a.r0 + a.ta - 1) / a.ta;
-                e = dispatch_short(b.wb, a, row_tiles * a.n_col_tiles, (size_t)a.ta * wst * ROW_BYTES, st);
+                e = dispatch_short(b.wb, a, row_tiles * a.n_col_tiles, (size_t)a.ta * wst * ROW_BYTES, st, n_launched > 0);
             } else {
                 a.ta = 1;
-                e = dispatch_long(b.wb, ctx->large_cw, a, (a.r1 - a.r0) * a.n_col_tiles, (size_t)wst * ROW_BYTES, st);
+                e = dispatch_long(b.wb, ctx->large_cw, a, (a.r1 - a.r0) * a.n_col_tiles, (size_t)wst * ROW_BYTES, st, n_launched > 0);
             }
             if (e != cudaSuccess) return cuda_fail(e, "sweep kernel launch");
-            ctx->launches++;
+            ctx->launches++; ++n_launched;
         }
     }
     return FAMSA_OK;
