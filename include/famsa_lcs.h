@@ -120,6 +120,52 @@ int64_t famsa_launch_count(const famsa_ctx* ctx);
  */
 int famsa_alu_peak(int device, double* instr_per_s, double* instr_per_clk_sm, double* sm_mhz);
 
+
+/* ---------------------------------------------------------------------------------------------
+ * Stage II consumer: the single-linkage guide tree over the similarities,
+ * built incrementally from the streamed row blocks in O(k) memory ("it can be
+ * computed incrementally, i.e., without storing the complete similarity matrix ... first two stages
+ * of FAMSA are performed simultaneously").  The paper uses SLINK, whose row update is a serial
+ * pointer chase; here the state is the maximum spanning tree of the rows consumed so far (the
+ * single-linkage dendrogram is its edges taken by decreasing similarity) and a row block is merged
+ * in by data-parallel Boruvka rounds over (old tree edges + the block's dense rows).  Under ties in
+ * the similarities the tree is not unique; the sorted merge similarities are.
+ */
+typedef struct famsa_tree famsa_tree;
+
+/* O(k) device state for k leaves on CUDA device `device`. */
+int famsa_tree_create(int64_t k, int device, famsa_tree** out);
+
+/*
+ * Consume rows [i0, i1) (i0 must equal the number of rows consumed so far; rows arrive in order).
+ *   sim_block  DEVICE  famsa_rows_pairs(i0, i1) floats in the famsa_lcs_rows layout, similarities >= 0
+ *                      (+inf allowed).  Read on `cuda_stream`; the call returns when the block has
+ *                      been merged (it synchronises that stream once per Boruvka round).
+ */
+int famsa_tree_update(famsa_tree* t, int64_t i0, int64_t i1, const float* sim_block, void* cuda_stream);
+
+/* HOST outputs, rows_consumed-1 entries each: the current spanning-tree edges (a > b, leaf indices). */
+int famsa_tree_edges(famsa_tree* t, int64_t* a_host, int64_t* b_host, float* sim_host);
+
+/*
+ * The dendrogram, k-1 merges by decreasing similarity (ties: by ascending (a, b) of the tree edge):
+ * merge t joins clusters id_a[t] < id_b[t] into cluster k + t (leaves are 0..k-1, scipy convention);
+ * sim[t] is the merge similarity, size[t] the leaves in the new cluster.  HOST outputs, k-1 entries.
+ * All k rows must have been consumed.
+ */
+int famsa_tree_finish(famsa_tree* t, int64_t* id_a_host, int64_t* id_b_host, float* sim_host, int64_t* size_host);
+
+void famsa_tree_free(famsa_tree* t);
+
+/*
+ * famsa_guide_tree -- stages I and II together, as the paper runs them: sweeps the
+ * packed set in row blocks of `block_rows` rows (0 = default 1024) and feeds each block to the tree
+ * while the next block is being swept on a second stream; row blocks never leave the device.
+ * Outputs as famsa_tree_finish, in SORTED leaf indices (map through famsa_perm).
+ */
+int famsa_guide_tree(famsa_ctx* ctx, int64_t block_rows, int64_t* id_a_host, int64_t* id_b_host,
+                     float* sim_host, int64_t* size_host);
+
 /* Tuning knob (process-wide, tests sweep it): rows of A per CTA on the register path, 1..12. */
 int famsa_set_tuning(int rows_per_cta);
 

@@ -17,7 +17,9 @@ FAMSA_MAX_LEN = 65535
 
 EXPORTS = ["famsa_pack", "famsa_lcs_rows", "famsa_lcs_rows_host", "famsa_rows_pairs", "famsa_rows_cells",
            "famsa_k", "famsa_perm", "famsa_lengths", "famsa_codes", "famsa_match", "famsa_launch_count",
-           "famsa_alu_peak", "famsa_set_tuning", "famsa_free", "famsa_strerror", "famsa_last_error"]
+           "famsa_alu_peak", "famsa_set_tuning", "famsa_free", "famsa_strerror", "famsa_last_error",
+           "famsa_tree_create", "famsa_tree_update", "famsa_tree_edges", "famsa_tree_finish", "famsa_tree_free",
+           "famsa_guide_tree"]
 
 
 class FamsaError(RuntimeError):
@@ -66,6 +68,18 @@ def lib():
         L.famsa_set_tuning.argtypes = [i32]
         L.famsa_free.restype = None
         L.famsa_free.argtypes = [vp]
+        L.famsa_tree_create.restype = i32
+        L.famsa_tree_create.argtypes = [i64, i32, ctypes.POINTER(vp)]
+        L.famsa_tree_update.restype = i32
+        L.famsa_tree_update.argtypes = [vp, i64, i64, vp, vp]
+        L.famsa_tree_edges.restype = i32
+        L.famsa_tree_edges.argtypes = [vp, vp, vp, vp]
+        L.famsa_tree_finish.restype = i32
+        L.famsa_tree_finish.argtypes = [vp, vp, vp, vp, vp]
+        L.famsa_tree_free.restype = None
+        L.famsa_tree_free.argtypes = [vp]
+        L.famsa_guide_tree.restype = i32
+        L.famsa_guide_tree.argtypes = [vp, i64, vp, vp, vp, vp]
         L.famsa_strerror.restype = ctypes.c_char_p
         L.famsa_strerror.argtypes = [i32]
         L.famsa_last_error.restype = ctypes.c_char_p
@@ -208,3 +222,69 @@ def famsa_alu_peak(device=0):
 
 def famsa_set_tuning(rows_per_cta):
     _check(lib().famsa_set_tuning(int(rows_per_cta)))
+
+
+# ---- stage II consumer: single-linkage guide tree (include/famsa_lcs.h) ----------------------------
+class Tree:
+    """Owns a famsa_tree*."""
+
+    def __init__(self, handle, k):
+        self.handle, self.k, self.rows = handle, int(k), 0
+
+    def free(self):
+        if self.handle:
+            lib().famsa_tree_free(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.free()
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+def famsa_tree_create(k, device=0):
+    out = ctypes.c_void_p()
+    _check(lib().famsa_tree_create(int(k), int(device), ctypes.byref(out)))
+    return Tree(out.value, k)
+
+
+def famsa_tree_update(tree, i0, i1, sim_block, cuda_stream=None):
+    """sim_block: float32 CUDA tensor in the famsa_lcs_rows layout for rows [i0, i1)."""
+    if cuda_stream is None:
+        import torch
+        cuda_stream = torch.cuda.current_stream().cuda_stream
+    elif hasattr(cuda_stream, "cuda_stream"):
+        cuda_stream = cuda_stream.cuda_stream
+    if sim_block is not None:
+        assert sim_block.is_cuda and sim_block.is_contiguous() and sim_block.element_size() == 4
+        assert sim_block.numel() >= famsa_rows_pairs(i0, i1)
+    _check(lib().famsa_tree_update(tree.handle, int(i0), int(i1), _ptr(sim_block), cuda_stream))
+    tree.rows = int(i1)
+
+
+def famsa_tree_edges(tree):
+    m = max(tree.rows - 1, 0)
+    a, b, w = np.empty(m, np.int64), np.empty(m, np.int64), np.empty(m, np.float32)
+    _check(lib().famsa_tree_edges(tree.handle, a.ctypes.data, b.ctypes.data, w.ctypes.data))
+    return a, b, w
+
+
+def famsa_tree_finish(tree):
+    m = max(tree.k - 1, 0)
+    a, b, w, s = np.empty(m, np.int64), np.empty(m, np.int64), np.empty(m, np.float32), np.empty(m, np.int64)
+    _check(lib().famsa_tree_finish(tree.handle, a.ctypes.data, b.ctypes.data, w.ctypes.data, s.ctypes.data))
+    return a, b, w, s
+
+
+def famsa_guide_tree(ctx, block_rows=0):
+    m = max(famsa_k(ctx) - 1, 0)
+    a, b, w, s = np.empty(m, np.int64), np.empty(m, np.int64), np.empty(m, np.float32), np.empty(m, np.int64)
+    _check(lib().famsa_guide_tree(ctx.handle, int(block_rows), a.ctypes.data, b.ctypes.data, w.ctypes.data, s.ctypes.data))
+    return a, b, w, s
