@@ -54,6 +54,8 @@ def parse_args():
     ap.add_argument("--full", action="store_true", help="a step is the full sweep whatever the config")
     ap.add_argument("--no-full", action="store_true", help="skip the extra single full sweep")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--guide-tree", action="store_true",
+                    help="also time stages I+II fused (famsa_guide_tree: full sweep + single-linkage tree), N=1 only")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU work per oracle sample")
     return ap.parse_args()
 
@@ -298,6 +300,21 @@ def run_cuda(args, rank, world, local_rank):
         fcells = F.famsa_rows_cells(ctx, 0, k)
         full = {"ms": fms, "gcups": fcells / fms / 1e6, "pairs": F.famsa_rows_pairs(0, k),
                 "pairs_per_s": F.famsa_rows_pairs(0, k) / fms * 1e3, "cells": fcells}
+    tree = None
+    if args.guide_tree and world == 1:
+        bufs = None
+        torch.cuda.empty_cache()
+        torch.cuda.synchronize()
+        l1 = F.famsa_launch_count(ctx)
+        t0 = time.perf_counter()
+        ia, ib, mw, msize = F.famsa_guide_tree(ctx, BLOCK_ROWS)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        fcells = F.famsa_rows_cells(ctx, 0, k)
+        tree = {"seconds": dt, "gcups_equivalent": fcells / dt / 1e9, "launches": F.famsa_launch_count(ctx) - l1,
+                "merges": int(mw.size), "top_similarity": float(mw[0]) if mw.size else None,
+                "last_similarity": float(mw[-1]) if mw.size else None,
+                "what": "famsa_guide_tree: full sweep (fp32 similarity only) + incremental single-linkage tree + dendrogram, wall clock"}
     peak1 = F.famsa_alu_peak(local_rank)
     ctx.free()
     if rank != 0:
@@ -360,6 +377,8 @@ def run_cuda(args, rank, world, local_rank):
     }
     if full is not None:
         line["full_sweep"] = full
+    if tree is not None:
+        line["guide_tree"] = tree
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
