@@ -130,21 +130,91 @@ __device__ __forceinline__ void store_pair(const SweepArgs& a, uint32_t i, uint3
 }
 
 // ---- register path: every row of the launch fits one block of W words --------------------------
+// Two rows per thread at once (NR = 2) while 2W words of V fit comfortably in registers: both rows
+// see the same residue, so the address PRMT and the residue-stream loads are shared and the two
+// carry chains are independent (more ILP per warp).
+#ifndef FAMSA_NR_POLICY
+#define FAMSA_NR_POLICY 2
+#endif
+__host__ __device__ constexpr int rows_per_thread(int w) {
+#if FAMSA_NR_POLICY == 0
+    return w <= 16 ? 2 : 1;
+#elif FAMSA_NR_POLICY == 1
+    return w <= 6 ? 4 : (w <= 10 ? 3 : (w <= 16 ? 2 : 1));
+#elif FAMSA_NR_POLICY == 2
+    return w <= 8 ? 3 : (w <= 16 ? 2 : 1);
+#elif FAMSA_NR_POLICY == 3
+    return w <= 4 ? 4 : (w <= 7 ? 3 : (w <= 20 ? 2 : 1));
+#else
+    return 1;
+#endif
+}
+
+template <int W, int NR, int TS>
+__device__ __forceinline__ void residue_step_rows(uint32_t (&V)[NR][W], uint32_t addr) {
+    uint32_t m[NR][W], s[NR][W];
+#pragma unroll
+    for (int p = 0; p < NR; ++p) LoadWords<W>::run(m[p], addr + p * TS);
+#pragma unroll
+    for (int p = 0; p < NR; ++p) {
+#pragma unroll
+        for (int w = 0; w < W; ++w) {
+            uint32_t u = V[p][w] & m[p][w];
+            if (w == 0) asm volatile("add.cc.u32 %0, %1, %2;" : "=r"(s[p][w]) : "r"(V[p][w]), "r"(u));
+            else        asm volatile("addc.cc.u32 %0, %1, %2;" : "=r"(s[p][w]) : "r"(V[p][w]), "r"(u));
+        }
+    }
+#pragma unroll
+    for (int p = 0; p < NR; ++p)
+#pragma unroll
+        for (int w = 0; w < W; ++w) V[p][w] = s[p][w] | (V[p][w] & ~m[p][w]);
+}
+
+template <int W, int NR, int TS>
+__device__ __forceinline__ void word_step_rows(uint32_t (&V)[NR][W], uint32_t bword, uint32_t tbase) {
+    residue_step_rows<W, NR, TS>(V, residue_addr<0>(bword, tbase));
+    residue_step_rows<W, NR, TS>(V, residue_addr<1>(bword, tbase));
+    residue_step_rows<W, NR, TS>(V, residue_addr<2>(bword, tbase));
+    residue_step_rows<W, NR, TS>(V, residue_addr<3>(bword, tbase));
+}
+
+template <int W, int NR, int TS>
+__device__ __forceinline__ void sweep_rows_block(uint32_t (&V)[NR][W], const uint4* __restrict__ bp, uint32_t nwords, uint32_t tbase) {
+    const uint32_t nfull = nwords >> 2, tail = nwords & 3;
+    uint4 cur = nwords ? __ldg(bp) : make_uint4(0, 0, 0, 0);
+    for (uint32_t c = 0; c < nfull; ++c) {
+        uint4 nxt = cur;
+        if ((c + 1) * 4 < nwords) nxt = __ldg(bp + (size_t)(c + 1) * GROUP);
+        word_step_rows<W, NR, TS>(V, cur.x, tbase);
+        word_step_rows<W, NR, TS>(V, cur.y, tbase);
+        word_step_rows<W, NR, TS>(V, cur.z, tbase);
+        word_step_rows<W, NR, TS>(V, cur.w, tbase);
+        cur = nxt;
+    }
+#pragma unroll 1
+    for (uint32_t q = 0; q < tail; ++q)                    // last, partial chunk: 1-3 words
+        word_step_rows<W, NR, TS>(V, q == 0 ? cur.x : (q == 1 ? cur.y : cur.z), tbase);
+}
+
 template <int W>
 __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
     extern __shared__ __align__(256) uint8_t smem[];
     asm volatile("griddepcontrol.launch_dependents;");
     constexpr int WST = (W + 1) & ~1;
+    constexpr int TS = WST * ROW_BYTES;                  // bytes between the tables of consecutive rows
+    constexpr int NR = rows_per_thread(W);
     const uint32_t col_tile = blockIdx.x % a.n_col_tiles, row_tile = blockIdx.x / a.n_col_tiles;
     const uint32_t r_lo = a.r0 + row_tile * a.ta;
     const uint32_t r_hi = min(r_lo + a.ta, a.r1);
     const uint32_t j0 = col_tile * TB;
     if (j0 + 1 >= r_hi) return;                          // whole tile on or above the diagonal
-    // stage the tile's tables: rows r_lo..r_hi-1 are contiguous (same stride WST each)
+    // stage the tile's tables: rows r_lo..r_hi-1 are contiguous (same stride each).  With NR > 1 the
+    // last step of a warp may run past row r_hi-1: the launch allocates NR-1 extra table slots, whose
+    // (uninitialised) content feeds V's that are never stored.
     {
         const uint4* src = a.tables + (size_t)a.toff[r_lo] * (ROW_BYTES / 16);
         uint4* dst = reinterpret_cast<uint4*>(smem);
-        const uint32_t n16 = (r_hi - r_lo) * WST * (ROW_BYTES / 16);
+        const uint32_t n16 = (r_hi - r_lo) * (TS / 16);
         for (uint32_t t = threadIdx.x; t < n16; t += TB) dst[t] = __ldg(src + t);
     }
     __syncthreads();
@@ -152,21 +222,26 @@ __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
     const uint32_t jw = j0 + (threadIdx.x & ~31u);       // first column of this warp
     if (jw + 1 >= r_hi) return;                          // this warp's columns are all >= every row (no barrier follows)
     const uint32_t j = jw + lane;
-    const uint32_t g = jw / GROUP;                       // jw < k, so g is a real group
-    const uint32_t gb = a.goff[g];
+    const uint32_t gb = a.goff[jw / GROUP];              // jw < k, so this is a real group
     const uint4* bp = a.stream + (size_t)gb * GROUP + lane;
     const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
     const uint32_t lb = j < r_hi ? a.len[j] : 0;         // columns >= r_hi are never stored
     const uint32_t nwords = (a.len[jw] + 3) >> 2;        // 4-residue words to sweep: jw is the group's longest sequence
-    for (uint32_t i = max(r_lo, jw + 1); i < r_hi; ++i) {
-        uint32_t V[W];
+    for (uint32_t i = max(r_lo, jw + 1); i < r_hi; i += NR) {   // rows NR at a time, from the first one below column jw
+        uint32_t V[NR][W];
 #pragma unroll
-        for (int w = 0; w < W; ++w) V[w] = 0xFFFFFFFFu;
-        sweep_block<W, false>(V, bp, nwords, smem_base + (i - r_lo) * (WST * ROW_BYTES), nullptr, false, false);
-        uint32_t lcs = 0;
+        for (int p = 0; p < NR; ++p)
 #pragma unroll
-        for (int w = 0; w < W; ++w) lcs += __popc(~V[w]);
-        if (j < i) store_pair(a, i, j, a.len[i], lb, lcs);
+            for (int w = 0; w < W; ++w) V[p][w] = 0xFFFFFFFFu;
+        sweep_rows_block<W, NR, TS>(V, bp, nwords, smem_base + (i - r_lo) * TS);
+#pragma unroll
+        for (int p = 0; p < NR; ++p) {
+            uint32_t lcs = 0;
+#pragma unroll
+            for (int w = 0; w < W; ++w) lcs += __popc(~V[p][w]);
+            const uint32_t row = i + p;
+            if (row < r_hi && j < row) store_pair(a, row, j, a.len[row], lb, lcs);
+        }
     }
 }
 
@@ -278,9 +353,10 @@ int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim
             const int wst = (b.wb + 1) & ~1;
             cudaError_t e;
             if (b.nblk == 1) {
-                a.ta = g_rows_per_cta;
+                const uint32_t nr = (uint32_t)rows_per_thread(b.wb);
+                a.ta = ((g_rows_per_cta + nr - 1) / nr) * nr;       // a whole number of NR-row steps per CTA
                 unsigned row_tiles = (a.r1 - a.r0 + a.ta - 1) / a.ta;
-                e = dispatch_short(b.wb, a, row_tiles * a.n_col_tiles, (size_t)a.ta * wst * ROW_BYTES, st, n_launched > 0);
+                e = dispatch_short(b.wb, a, row_tiles * a.n_col_tiles, (size_t)(a.ta + nr - 1) * wst * ROW_BYTES, st, n_launched > 0);
             } else {
                 a.ta = 1;
                 e = dispatch_long(b.wb, ctx->large_cw, a, (a.r1 - a.r0) * a.n_col_tiles, (size_t)wst * ROW_BYTES, st, n_launched > 0);
