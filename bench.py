@@ -330,6 +330,16 @@ def run_cuda(args, rank, world, local_rank):
         cpu = {"value": ccells / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
                "pairs_per_s": pi.size / dt,
                "sample": "%d seeded uniform pairs of the step's row blocks (%.3g cells, %.1f s)" % (pi.size, ccells, dt)}
+    cpu_bp = None
+    if not args.no_cpu:
+        from oracle import famsa_oracle
+        pi, pj, ccells, cores = oracle_sample(seqs, offsets, blocks, args.cpu_seconds * 6, seed=11)   # ~10x faster than the DP
+        t0 = time.perf_counter()
+        famsa_oracle.bitpar_pairs(seqs, offsets, pi, pj)
+        dt = time.perf_counter() - t0
+        cpu_bp = {"value": ccells / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "context: the paper's own CPU design "
+                  "(64-bit bit-parallel LCS, one pair per task over threads, scalar; oracle/bitpar_cpu.c) -- not a parity oracle",
+                  "pairs_per_s": pi.size / dt, "sample": "%d seeded uniform pairs (%.3g cells, %.1f s)" % (pi.size, ccells, dt)}
     p_int = max(peak0["instr_per_s"], peak1["instr_per_s"])          # measured INT32 ALU-pipe rate (thread-instr/s)
     sm_count = torch.cuda.get_device_properties(local_rank).multi_processor_count
     achieved = cells_step * args.steps * ALU_INSTR_PER_CELL / (ev[0].elapsed_time(ev[-1]) * 1e-3)   # this rank's stream
@@ -373,6 +383,7 @@ def run_cuda(args, rank, world, local_rank):
         "gpu_launches": launches,
         "roofline": roofline,
         "cpu_baseline": cpu,
+        "cpu_bitparallel": cpu_bp,
         "output_gb_per_s": pairs_all * args.steps * (2 + (4 if want_sim else 0)) / sec / 1e9,
     }
     if full is not None:

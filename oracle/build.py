@@ -8,16 +8,17 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "lcs_oracle.c")
+SRC_BITPAR = os.path.join(HERE, "bitpar_cpu.c")   # context baseline, not an oracle (see its header)
 LIB = os.path.join(HERE, "libfamsa_oracle.so")
 
 
 def build(force: bool = False) -> str:
     if (not force and os.path.exists(LIB)
-            and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
+            and os.path.getmtime(LIB) >= max(os.path.getmtime(SRC), os.path.getmtime(SRC_BITPAR))):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
-    subprocess.check_call(["gcc", "-O2", "-std=c99", "-Wall", "-shared", "-fPIC",
-                           "-pthread", SRC, "-o", tmp, "-lm"])
+    subprocess.check_call(["gcc", "-O2", "-std=gnu99", "-Wall", "-shared", "-fPIC",
+                           "-pthread", SRC, SRC_BITPAR, "-o", tmp, "-lm"])
     os.replace(tmp, LIB)
     return LIB
 

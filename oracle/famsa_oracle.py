@@ -41,6 +41,9 @@ def _load():
         lib.oracle_pairs.argtypes = [u8p, i64p, i64p, i64p, ctypes.c_int64,
                                      ctypes.POINTER(ctypes.c_int32),
                                      ctypes.POINTER(ctypes.c_double), ctypes.c_int32]
+        lib.bitpar_pairs.restype = ctypes.c_int
+        lib.bitpar_pairs.argtypes = [u8p, i64p, i64p, i64p, ctypes.c_int64, ctypes.c_int32,
+                                     ctypes.POINTER(ctypes.c_int32), ctypes.c_int32]
         _lib = lib
     return _lib
 
@@ -133,3 +136,19 @@ def rows(seqs, offsets, i0, i1, want_sim=True, n_threads=None):
     row_start = ii * (ii - 1) // 2 - i0 * (i0 - 1) // 2
     jj = np.arange(ii.size, dtype=np.int64) - row_start
     return pairs(seqs, offsets, perm[ii], perm[jj], want_sim, n_threads)
+
+
+def bitpar_pairs(seqs, offsets, pi, pj, n_threads=None):
+    """CONTEXT BASELINE, not an oracle: the paper's own CPU design (64-bit bit-parallel LCS, one pair
+    per task over threads; oracle/bitpar_cpu.c).  LCS (int32) for pairs in ORIGINAL index space."""
+    codes, cp = _u8(encode(seqs))
+    offsets, op = _i64(offsets)
+    pi, pip = _i64(pi)
+    pj, pjp = _i64(pj)
+    lcs = np.empty(pi.size, dtype=np.int32)
+    if n_threads is None:
+        n_threads = n_threads_default()
+    max_len = int(np.diff(offsets).max()) if offsets.size > 1 else 0
+    _load().bitpar_pairs(cp, op, pip, pjp, pi.size, max_len,
+                         lcs.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), int(n_threads))
+    return lcs
