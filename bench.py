@@ -31,7 +31,7 @@ sys.path.insert(0, ROOT)
 METRIC = "all_pairs_lcs_gcups"
 UNIT = "GCUPS"
 BLOCK_ROWS = 1024
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 2.098e9   # profiles/r01_ncu_sweep_short_w10_config4.md (ncu --set full, one launch)
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 3.387e9   # profiles/r01_ncu_sweep_short_v2_config4.md (ncu --set full, one <10> launch)
 ALU_INSTR_PER_CELL = 3.0 / 32.0      # LOP3 + IADD3.X + LOP3 per 32-bit word-step
 WORKLOADS = {
     0: "configs[0]: k=500, one family, all 124750 pairs",
@@ -352,7 +352,7 @@ def run_cuda(args, rank, world, local_rank):
         "bound": "alu", "achieved": achieved / 1e12, "peak": p_int / 1e12, "unit": "TIOP/s (int32 ALU-pipe lane-instr)",
         "frac": achieved / p_int, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
         "traffic_note": "dram__bytes_read+write of ONE sweep_short_kernel<10> launch (1.68e8 pairs of configs[4]), "
-                        "from profiles/r01_ncu_sweep_short_w10_config4.md; not measured in this run",
+                        "from profiles/r01_ncu_sweep_short_v2_config4.md; not measured in this run",
         "kernel": "famsa::sweep_short_kernel<W> (%d launches per step)" % (launches // max(args.steps, 1)),
         "algorithmic_instr_per_cell": ALU_INSTR_PER_CELL,
         "peak_source": "famsa_alu_peak micro-kernel, measured in this run (MEASURED_PEAKS.json has no integer peak)",

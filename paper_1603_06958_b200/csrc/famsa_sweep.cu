@@ -395,7 +395,11 @@ extern "C" int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1, uint1
     if (famsa_rows_pairs(i0, i1) == 0) return FAMSA_OK;
     FAMSA_CUDA(cudaSetDevice(ctx->device));
     // lazily create the ping-pong staging (two row-block buffers of up to 32 Mi pairs each)
-    const size_t want = (size_t)std::min<int64_t>(famsa_rows_pairs(i0, i1), (int64_t)32 << 20);
+    // chunk size: about 1/8 of the call (so the copy of chunk n overlaps the sweep of chunk n+1),
+    // between 1 Mi and 32 Mi pairs, and never smaller than the longest row
+    const int64_t total_pairs = famsa_rows_pairs(i0, i1);
+    const int64_t chunk_pairs = std::max<int64_t>(std::min<int64_t>(std::max<int64_t>(total_pairs / 8, (int64_t)1 << 20), (int64_t)32 << 20), i1);
+    const size_t want = (size_t)std::min<int64_t>(total_pairs, chunk_pairs);
     if (!ctx->s_compute) {
         FAMSA_CUDA(cudaStreamCreateWithFlags(&ctx->s_compute, cudaStreamNonBlocking));
         FAMSA_CUDA(cudaStreamCreateWithFlags(&ctx->s_copy, cudaStreamNonBlocking));
@@ -424,7 +428,7 @@ extern "C" int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1, uint1
     int64_t r = i0; int n = 0; int64_t done_pairs = 0;
     while (r < i1) {
         int64_t e = r + 1;
-        while (e < i1 && famsa_rows_pairs(r, e + 1) <= (int64_t)ctx->buf_pairs) ++e;
+        while (e < i1 && famsa_rows_pairs(r, e + 1) <= (int64_t)want) ++e;
         const int64_t np = famsa_rows_pairs(r, e);
         if (np > (int64_t)ctx->buf_pairs) { set_error("famsa_lcs_rows_host: a single row exceeds the staging buffer"); return FAMSA_ENOMEM; }
         const int b = n & 1;

@@ -228,3 +228,48 @@ def test_planted_long(F):
         lcs, sim = gpu_rows(F, ctx, 0, 2)
     assert lcs[0] == p
     assert sim[0] == pytest.approx(p / float(3900 + 3500 - 2 * p) ** 2, rel=1e-6)
+
+
+def test_random_sets(F, oracle):
+    """Seeded random sets: ragged lengths 1..1300 (register path, every rows-per-thread variant, and the
+    blocked path), alphabets of 2-25 letters, set sizes that leave partial warps and partial row steps."""
+    rng = np.random.default_rng(101)
+    for trial in range(6):
+        k = int(rng.integers(2, 140))
+        sigma = int(rng.choice([2, 4, 20, 25]))
+        hi = int(rng.choice([40, 300, 700, 1300]))
+        seq_list = [rng.integers(0, sigma, int(rng.integers(1, hi + 1))).astype(np.uint8) for _ in range(k)]
+        if trial % 2:
+            seq_list[int(rng.integers(0, k))] = seq_list[0].copy()        # an exact duplicate
+        seqs, offsets = make_set(seq_list)
+        check_all_rows(F, oracle, seqs, offsets)
+
+
+def test_two_streams_one_ctx(F, oracle):
+    """One ctx serves concurrent famsa_lcs_rows calls on different streams (it is read-only after pack)."""
+    import torch
+    from paper_1603_06958_b200 import synth
+    seqs, offsets = synth.family(1, k=900, seed=55)
+    k = 900
+    with F.famsa_pack(seqs, offsets) as ctx:
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        n1, n2 = F.famsa_rows_pairs(0, 600), F.famsa_rows_pairs(600, k)
+        l1 = torch.zeros(n1, dtype=torch.uint16, device="cuda"); f1 = torch.zeros(n1, dtype=torch.float32, device="cuda")
+        l2 = torch.zeros(n2, dtype=torch.uint16, device="cuda"); f2 = torch.zeros(n2, dtype=torch.float32, device="cuda")
+        torch.cuda.synchronize()
+        for _ in range(3):
+            F.famsa_lcs_rows(ctx, 0, 600, l1, f1, s1)
+            F.famsa_lcs_rows(ctx, 600, k, l2, f2, s2)
+        torch.cuda.synchronize()
+        lcs = np.concatenate([l1.cpu().numpy(), l2.cpu().numpy()]).astype(np.int64)
+        sim = np.concatenate([f1.cpu().numpy(), f2.cpu().numpy()])
+    lref, sref = oracle.rows(seqs, offsets, 0, k)
+    assert_match(lcs, sim, lref, sref)
+
+
+def test_alu_peak_is_sane(F):
+    """The roofline denominator: the ALU pipe issues 64 thread-instructions per clock per SM on sm_100."""
+    p = F.famsa_alu_peak(0)
+    assert 55.0 < p["instr_per_clk_sm"] <= 64.5
+    assert 1000.0 < p["sm_mhz"] < 2300.0
+    assert p["instr_per_s"] == pytest.approx(p["instr_per_clk_sm"] * p["sm_mhz"] * 1e6 * 148, rel=0.05)
