@@ -257,13 +257,20 @@ def run_cuda(args, rank, world, local_rank):
     value = cells_all * args.steps / sec / 1e9
 
     # ---- e2e: HOST buffers through the C ABI; pack (H2D of the residues) + sweep + D2H every step
-    h_lcs = torch.empty(max_pairs, dtype=torch.uint16).pin_memory()
-    h_sim = torch.empty(max_pairs, dtype=torch.float32).pin_memory() if want_sim else None
+    # (one call over all rows when the whole result fits 2 GB of pinned memory, else one call per row block
+    #  into a reused pinned row-block buffer -- the consumer owns a block only until the next one arrives)
+    one_call = stride == 1 and pairs_step * 6 <= 2e9
+    e2e_pairs = pairs_step if one_call else max_pairs
+    h_lcs = torch.empty(e2e_pairs, dtype=torch.uint16).pin_memory()
+    h_sim = torch.empty(e2e_pairs, dtype=torch.float32).pin_memory() if want_sim else None
     e2e_steps = max(1, min(args.steps, 2))
     def e2e_step():
         c2 = F.famsa_pack(seqs, offsets, device=local_rank)
-        for a, b in blocks:
-            F.famsa_lcs_rows_host(c2, a, b, h_lcs, h_sim)
+        if one_call:
+            F.famsa_lcs_rows_host(c2, 0, k, h_lcs, h_sim)
+        else:
+            for a, b in blocks:
+                F.famsa_lcs_rows_host(c2, a, b, h_lcs, h_sim)
         c2.free()
     e2e_step()                                                # warm-up (allocations, staging buffers)
     barrier()

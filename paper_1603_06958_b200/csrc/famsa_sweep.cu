@@ -34,6 +34,24 @@ struct SweepArgs {
     uint32_t        nblk;        // table blocks per row (1 on the register path)
 };
 
+// ---- table staging: one TMA bulk copy (cp.async.bulk, global -> shared) per tile, completion on an
+// mbarrier; no registers or LSU instructions are spent on it and the waiting warps sleep on the barrier.
+__device__ __forceinline__ void mbar_init(uint32_t bar) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(bar));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");        // earlier generic reads of dst vs. this async write
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\t"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+                 "@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}" :: "r"(bar), "r"(parity) : "memory");
+}
+
 template <int IMM>
 __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
     uint32_t v;
@@ -211,22 +229,21 @@ __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
     // stage the tile's tables: rows r_lo..r_hi-1 are contiguous (same stride each).  With NR > 1 the
     // last step of a warp may run past row r_hi-1: the launch allocates NR-1 extra table slots, whose
     // (uninitialised) content feeds V's that are never stored.
-    {
-        const uint4* src = a.tables + (size_t)a.toff[r_lo] * (ROW_BYTES / 16);
-        uint4* dst = reinterpret_cast<uint4*>(smem);
-        const uint32_t n16 = (r_hi - r_lo) * (TS / 16);
-        for (uint32_t t = threadIdx.x; t < n16; t += TB) dst[t] = __ldg(src + t);
-    }
+    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);   // 256-byte aligned: no static shared memory
+    const uint32_t mbar = smem_base + (a.ta + NR - 1) * TS;                  // the mbarrier sits after the table slots
+    if (threadIdx.x == 0) mbar_init(mbar);
     __syncthreads();
+    if (threadIdx.x == 0)
+        bulk_load(smem_base, a.tables + (size_t)a.toff[r_lo] * (ROW_BYTES / 16), (r_hi - r_lo) * TS, mbar);
     const uint32_t lane = threadIdx.x & 31;
     const uint32_t jw = j0 + (threadIdx.x & ~31u);       // first column of this warp
     if (jw + 1 >= r_hi) return;                          // this warp's columns are all >= every row (no barrier follows)
     const uint32_t j = jw + lane;
     const uint32_t gb = a.goff[jw / GROUP];              // jw < k, so this is a real group
     const uint4* bp = a.stream + (size_t)gb * GROUP + lane;
-    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
     const uint32_t lb = j < r_hi ? a.len[j] : 0;         // columns >= r_hi are never stored
     const uint32_t nwords = (a.len[jw] + 3) >> 2;        // 4-residue words to sweep: jw is the group's longest sequence
+    mbar_wait(mbar, 0);                                  // the tables have landed
     for (uint32_t i = max(r_lo, jw + 1); i < r_hi; i += NR) {   // rows NR at a time, from the first one below column jw
         uint32_t V[NR][W];
 #pragma unroll
@@ -266,12 +283,12 @@ __global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
     unsigned short cv[CW * 2];                           // 16 carry bits per 16-residue chunk
     uint32_t lcs = 0;
     const uint4* src = a.tables + (size_t)a.toff[i] * (ROW_BYTES / 16);
+    const uint32_t mbar = smem_base + WST * ROW_BYTES;   // the mbarrier sits after the table block
+    if (threadIdx.x == 0) mbar_init(mbar);
     for (uint32_t blk = 0; blk < a.nblk; ++blk) {
-        if (blk) __syncthreads();                        // everyone done with the previous block
-        uint4* dst = reinterpret_cast<uint4*>(smem);
-        for (uint32_t t = threadIdx.x; t < WST * (ROW_BYTES / 16); t += TB)
-            dst[t] = __ldg(src + (size_t)blk * WST * (ROW_BYTES / 16) + t);
-        __syncthreads();
+        __syncthreads();                                 // barrier initialised / everyone done with the previous block
+        if (threadIdx.x == 0) bulk_load(smem_base, src + (size_t)blk * WST * (ROW_BYTES / 16), WST * ROW_BYTES, mbar);
+        mbar_wait(mbar, blk & 1);                        // phase flips once per block
         if (active) {
             uint32_t V[W];
 #pragma unroll
@@ -355,11 +372,12 @@ int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim
             if (b.nblk == 1) {
                 const uint32_t nr = (uint32_t)rows_per_thread(b.wb);
                 a.ta = ((g_rows_per_cta + nr - 1) / nr) * nr;       // a whole number of NR-row steps per CTA
+                while (a.ta > nr && (size_t)(a.ta + nr - 1) * wst * ROW_BYTES + 16 > 48 * 1024) a.ta -= nr;   // default dynamic smem limit
                 unsigned row_tiles = (a.r1 - a.r0 + a.ta - 1) / a.ta;
-                e = dispatch_short(b.wb, a, row_tiles * a.n_col_tiles, (size_t)(a.ta + nr - 1) * wst * ROW_BYTES, st, n_launched > 0);
+                e = dispatch_short(b.wb, a, row_tiles * a.n_col_tiles, (size_t)(a.ta + nr - 1) * wst * ROW_BYTES + 16, st, n_launched > 0);
             } else {
                 a.ta = 1;
-                e = dispatch_long(b.wb, ctx->large_cw, a, (a.r1 - a.r0) * a.n_col_tiles, (size_t)wst * ROW_BYTES, st, n_launched > 0);
+                e = dispatch_long(b.wb, ctx->large_cw, a, (a.r1 - a.r0) * a.n_col_tiles, (size_t)wst * ROW_BYTES + 16, st, n_launched > 0);
             }
             if (e != cudaSuccess) return cuda_fail(e, "sweep kernel launch");
             ctx->launches++; ++n_launched;
@@ -409,6 +427,10 @@ extern "C" int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1, uint1
         }
     }
     if (ctx->buf_pairs < want) {
+        // size the staging once per ctx (1/8 of the whole triangle, 1 Mi .. 32 Mi pairs, at least one row),
+        // so that a stream of growing row-block calls does not reallocate it
+        const int64_t tri = ctx->k * (ctx->k - 1) / 2;
+        const size_t cap = (size_t)std::max<int64_t>(std::max<int64_t>(std::min<int64_t>(std::max<int64_t>(tri / 8, (int64_t)1 << 20), (int64_t)32 << 20), ctx->k), (int64_t)want);
         FAMSA_CUDA(cudaDeviceSynchronize());
         for (int b = 0; b < 2; ++b) {
             cudaFree(ctx->d_lcs_buf[b]); cudaFree(ctx->d_sim_buf[b]);
@@ -416,13 +438,13 @@ extern "C" int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1, uint1
         }
         ctx->buf_pairs = 0;
         for (int b = 0; b < 2; ++b) {
-            cudaError_t e1 = cudaMalloc((void**)&ctx->d_lcs_buf[b], want * sizeof(uint16_t));
-            cudaError_t e2 = cudaMalloc((void**)&ctx->d_sim_buf[b], want * sizeof(float));
+            cudaError_t e1 = cudaMalloc((void**)&ctx->d_lcs_buf[b], cap * sizeof(uint16_t));
+            cudaError_t e2 = cudaMalloc((void**)&ctx->d_sim_buf[b], cap * sizeof(float));
             if (e1 != cudaSuccess || e2 != cudaSuccess) {
                 cudaGetLastError(); set_error("famsa_lcs_rows_host: device allocation failed"); return FAMSA_ENOMEM;
             }
         }
-        ctx->buf_pairs = want;
+        ctx->buf_pairs = cap;
     }
     // chunk the row range so that each chunk fits a buffer (a single row always fits: i < 2^32 / ... k <= buf)
     int64_t r = i0; int n = 0; int64_t done_pairs = 0;
