@@ -55,7 +55,7 @@ def parse_args():
     ap.add_argument("--no-full", action="store_true", help="skip the extra single full sweep")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--guide-tree", action="store_true",
-                    help="also time stages I+II fused (famsa_guide_tree: full sweep + single-linkage tree), N=1 only")
+                    help="also time stages I+II (full sweep + single-linkage guide tree), the whole job dealt over the ranks")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU work per oracle sample")
     return ap.parse_args()
 
@@ -195,6 +195,33 @@ def reduce_over_ranks(dist, ms, cells, pairs, device):
     return float(t.item()), float(tot[0].item()), float(tot[1].item())
 
 
+def gather_forests(dist, a, b, w, k, device):
+    """The one exchange step of the multi-GPU guide tree: every rank's forest edges (<= k-1 each) to every
+    rank.  Padded all_gather (NCCL on device tensors; gloo on CPU tensors in the tests).  Returns a list of
+    (a, b, w) numpy triples, one per rank."""
+    import torch
+    if dist is None:
+        return [(a, b, w)]
+    world = dist.get_world_size()
+    cap = max(int(k) - 1, 1)
+    ab = torch.zeros((cap, 2), dtype=torch.int64, device=device)
+    ww = torch.zeros(cap, dtype=torch.float32, device=device)
+    n = torch.tensor([a.size], dtype=torch.int64, device=device)
+    if a.size:
+        ab[:a.size, 0] = torch.from_numpy(np.ascontiguousarray(a)).to(device)
+        ab[:a.size, 1] = torch.from_numpy(np.ascontiguousarray(b)).to(device)
+        ww[:a.size] = torch.from_numpy(np.ascontiguousarray(w)).to(device)
+    abs_, wws, ns = ([torch.zeros_like(x) for _ in range(world)] for x in (ab, ww, n))
+    dist.all_gather(abs_, ab)
+    dist.all_gather(wws, ww)
+    dist.all_gather(ns, n)
+    out = []
+    for r in range(world):
+        m = int(ns[r].item())
+        out.append((abs_[r][:m, 0].cpu().numpy(), abs_[r][:m, 1].cpu().numpy(), wws[r][:m].cpu().numpy()))
+    return out
+
+
 def run_cuda(args, rank, world, local_rank):
     import torch
     from paper_1603_06958_b200 import famsa as F, synth
@@ -308,20 +335,37 @@ def run_cuda(args, rank, world, local_rank):
         full = {"ms": fms, "gcups": fcells / fms / 1e6, "pairs": F.famsa_rows_pairs(0, k),
                 "pairs_per_s": F.famsa_rows_pairs(0, k) / fms * 1e3, "cells": fcells}
     tree = None
-    if args.guide_tree and world == 1:
+    if args.guide_tree:
+        # stages I + II, the WHOLE job dealt over the ranks (strong scaling): rank r sweeps row blocks
+        # r, r + N, ... and keeps their spanning forest; one all_gather of the forests' edges; rank 0 merges
         bufs = None
         torch.cuda.empty_cache()
-        torch.cuda.synchronize()
+        barrier()
         l1 = F.famsa_launch_count(ctx)
         t0 = time.perf_counter()
-        ia, ib, mw, msize = F.famsa_guide_tree(ctx, BLOCK_ROWS)
-        torch.cuda.synchronize()
+        forest = F.famsa_guide_forest(ctx, BLOCK_ROWS, rank, world)
+        fa, fb, fw = F.famsa_tree_edges(forest)
+        parts = gather_forests(dist, fa, fb, fw, k, dev)
+        n_merges = 0
+        if rank == 0:
+            for r in range(1, world):
+                F.famsa_tree_merge_edges(forest, *parts[r])
+            ia, ib, mw, msize = F.famsa_tree_finish(forest)
+            n_merges = int(mw.size)
+        barrier()
         dt = time.perf_counter() - t0
+        forest.free()
+        if dist is not None:
+            tt = torch.tensor([dt], dtype=torch.float64, device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            dt = float(tt.item())
         fcells = F.famsa_rows_cells(ctx, 0, k)
-        tree = {"seconds": dt, "gcups_equivalent": fcells / dt / 1e9, "launches": F.famsa_launch_count(ctx) - l1,
-                "merges": int(mw.size), "top_similarity": float(mw[0]) if mw.size else None,
-                "last_similarity": float(mw[-1]) if mw.size else None,
-                "what": "famsa_guide_tree: full sweep (fp32 similarity only) + incremental single-linkage tree + dendrogram, wall clock"}
+        if rank == 0:
+            tree = {"seconds": dt, "gcups_equivalent": fcells / dt / 1e9, "launches_rank0": F.famsa_launch_count(ctx) - l1,
+                    "merges": n_merges, "top_similarity": float(mw[0]) if mw.size else None,
+                    "last_similarity": float(mw[-1]) if mw.size else None, "scaling": "strong", "n_gpus": world,
+                    "what": "famsa_guide_forest per rank (cyclic deal of all 1024-row blocks: sweep, fp32 similarity only, + incremental "
+                            "single-linkage forest), all_gather of the forests' edges, merge + dendrogram on rank 0; wall clock, max over ranks"}
     peak1 = F.famsa_alu_peak(local_rank)
     ctx.free()
     if rank != 0:

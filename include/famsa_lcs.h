@@ -137,21 +137,33 @@ typedef struct famsa_tree famsa_tree;
 int famsa_tree_create(int64_t k, int device, famsa_tree** out);
 
 /*
- * Consume rows [i0, i1) (i0 must equal the number of rows consumed so far; rows arrive in order).
+ * Consume rows [i0, i1) of the similarity matrix.  Row blocks may arrive in ANY order and each row
+ * once (the state is the maximum spanning forest of the entries seen so far), so a rank of a
+ * multi-GPU job can feed only the blocks it swept.
  *   sim_block  DEVICE  famsa_rows_pairs(i0, i1) floats in the famsa_lcs_rows layout, similarities >= 0
  *                      (+inf allowed).  Read on `cuda_stream`; the call returns when the block has
  *                      been merged (it synchronises that stream once per Boruvka round).
  */
 int famsa_tree_update(famsa_tree* t, int64_t i0, int64_t i1, const float* sim_block, void* cuda_stream);
 
-/* HOST outputs, rows_consumed-1 entries each: the current spanning-tree edges (a > b, leaf indices). */
+/*
+ * Merge m weighted edges (a[e], b[e], sim[e]) into the forest: MSF(E1 u E2) = MSF(MSF(E1) u MSF(E2)),
+ * so the forests of several ranks (famsa_tree_edges of each, gathered) merged into one tree give the
+ * tree of the whole matrix.  HOST inputs; leaves in [0, k), similarities >= 0.
+ */
+int famsa_tree_merge_edges(famsa_tree* t, const int64_t* a_host, const int64_t* b_host, const float* sim_host, int64_t m);
+
+/* Edges in the current forest (k-1 once every row has been consumed or merged in). */
+int64_t famsa_tree_edge_count(const famsa_tree* t);
+
+/* HOST outputs, famsa_tree_edge_count entries each: the current forest's edges (a > b, leaf indices). */
 int famsa_tree_edges(famsa_tree* t, int64_t* a_host, int64_t* b_host, float* sim_host);
 
 /*
  * The dendrogram, k-1 merges by decreasing similarity (ties: by ascending (a, b) of the tree edge):
  * merge t joins clusters id_a[t] < id_b[t] into cluster k + t (leaves are 0..k-1, scipy convention);
  * sim[t] is the merge similarity, size[t] the leaves in the new cluster.  HOST outputs, k-1 entries.
- * All k rows must have been consumed.
+ * Every row must have been consumed (or the missing ones merged in as edges): else FAMSA_ERANGE.
  */
 int famsa_tree_finish(famsa_tree* t, int64_t* id_a_host, int64_t* id_b_host, float* sim_host, int64_t* size_host);
 
@@ -165,6 +177,15 @@ void famsa_tree_free(famsa_tree* t);
  */
 int famsa_guide_tree(famsa_ctx* ctx, int64_t block_rows, int64_t* id_a_host, int64_t* id_b_host,
                      float* sim_host, int64_t* size_host);
+
+/*
+ * famsa_guide_forest -- the same pipeline over one part of the row blocks: blocks part, part + parts,
+ * part + 2*parts, ... (0 <= part < parts), the cyclic deal that balances the triangle over `parts`
+ * GPUs.  Returns the tree handle (its forest spans only what this part saw); gather every part's
+ * famsa_tree_edges, famsa_tree_merge_edges them into one tree and famsa_tree_finish it.
+ * The caller frees *out with famsa_tree_free.
+ */
+int famsa_guide_forest(famsa_ctx* ctx, int64_t block_rows, int64_t part, int64_t parts, famsa_tree** out);
 
 /* Tuning knob (process-wide, tests sweep it): rows of A per CTA on the register path, 1..12. */
 int famsa_set_tuning(int rows_per_cta);

@@ -19,7 +19,10 @@
 struct famsa_tree {
     int      device = 0;
     int64_t  k = 0;
-    int64_t  rows = 0;                 // rows consumed so far; T has max(rows-1, 0) edges
+    int64_t  rows = 0;                 // rows consumed so far (any order)
+    int64_t  max_row_end = 0;          // largest i1 seen: leaves 0..max_row_end-1 are one component
+    int64_t  m = 0;                    // edges of the current forest
+    bool     merged = false;           // sparse edges were merged in: components above max_row_end may exist
     uint32_t *ta[2] = {nullptr, nullptr}, *tb[2] = {nullptr, nullptr};   // tree edges, a > b (double buffer)
     float    *tw[2] = {nullptr, nullptr};
     int      cur = 0;
@@ -104,10 +107,12 @@ __global__ void __launch_bounds__(256) tree_col_kernel(const float* __restrict__
 namespace famsa {
 
 struct TreeArgs {
-    uint32_t n;                 // vertices after this update (= i1)
-    uint32_t i0, i1;
-    uint32_t m;                 // old tree edges (i0 - 1, or 0)
-    const uint32_t *ta, *tb; const float* tw;            // old tree
+    uint32_t n;                 // all k leaves
+    uint32_t i0, i1;            // rows of the dense block (i0 == i1: none)
+    uint32_t m;                 // edges of the current forest
+    uint32_t xm;                // extra sparse edges (famsa_tree_merge_edges)
+    const uint32_t *xa, *xb; const float* xw;
+    const uint32_t *ta, *tb; const float* tw;            // current forest
     uint32_t *na, *nb; float* nw;                        // new tree being recorded
     const uint32_t* comp; uint32_t* comp_next; uint32_t* parent;
     const float *cw_row, *cw_col; const uint32_t *co_row, *co_col;
@@ -128,7 +133,7 @@ __global__ void tree_reset_kernel(TreeArgs a, int first) {
     if (x == 0) { a.counters[1] = 0; if (first) a.counters[0] = 0; }
 }
 
-// Items: [0, n) row candidates, [n, 2n) column candidates, [2n, 2n+m) old tree edges.
+// Items: [0, n) row candidates, [n, 2n) column candidates, [2n, 2n+m) forest edges, then xm extra edges.
 // PASS 0: per component, the highest similarity of an outgoing edge.  PASS 1: among the edges that
 // reach it, the smallest edge id.  Together: the component's minimum-key outgoing edge.
 template <int PASS>
@@ -137,16 +142,21 @@ __global__ void tree_best_kernel(TreeArgs a) {
     uint32_t x, y; float w;
     bool both = false;
     if (t < a.n) {
-        if (t < a.i0) return;
+        if (t < a.i0 || t >= a.i1) return;
         x = t; w = a.cw_row[t]; y = a.co_row[t];
     } else if (t < 2 * a.n) {
         x = t - a.n;
-        if (x + 1 >= a.i1) return;
+        if (a.i1 == a.i0 || x + 1 >= a.i1) return;
         w = a.cw_col[x]; y = a.co_col[x];
     } else if (t < 2 * a.n + a.m) {
         const uint32_t e = t - 2 * a.n;
         x = a.ta[e]; y = a.tb[e]; w = a.tw[e];
         if (a.comp[x] == a.comp[y]) return;
+        both = true;
+    } else if (t < 2 * a.n + a.m + a.xm) {
+        const uint32_t e = t - 2 * a.n - a.m;
+        x = a.xa[e]; y = a.xb[e]; w = a.xw[e];
+        if (x == y || a.comp[x] == a.comp[y]) return;
         both = true;
     } else {
         return;
@@ -244,55 +254,111 @@ extern "C" int famsa_tree_create(int64_t k, int device, famsa_tree** out) {
     return FAMSA_OK;
 }
 
-extern "C" int famsa_tree_update(famsa_tree* t, int64_t i0, int64_t i1, const float* sim_block, void* cuda_stream) {
-    if (!t) { set_error("famsa_tree_update: tree is NULL"); return FAMSA_EINVAL; }
-    if (i0 != t->rows || i1 < i0 || i1 > t->k) {
-        set_error("famsa_tree_update: rows must arrive in order: expected i0 = " + std::to_string(t->rows)); return FAMSA_ERANGE;
-    }
-    if (i1 == i0) return FAMSA_OK;
-    if (!sim_block && famsa_rows_pairs(i0, i1) > 0) { set_error("famsa_tree_update: sim_block is NULL"); return FAMSA_EINVAL; }
-    FAMSA_CUDA(cudaSetDevice(t->device));
-    cudaStream_t st = (cudaStream_t)cuda_stream;
+namespace famsa {
+
+// Boruvka rounds over (current forest) + (dense block rows [i0, i1), if any) + (xm extra edges).
+static int tree_rounds(famsa_tree* t, int64_t i0, int64_t i1, const float* sim_block,
+                       const uint32_t* xa, const uint32_t* xb, const float* xw, uint32_t xm, cudaStream_t st) {
     const int cur = t->cur, nxt = cur ^ 1;
     TreeArgs a;
-    a.n = (uint32_t)i1; a.i0 = (uint32_t)i0; a.i1 = (uint32_t)i1; a.m = i0 > 0 ? (uint32_t)(i0 - 1) : 0;
+    a.n = (uint32_t)t->k; a.i0 = (uint32_t)i0; a.i1 = (uint32_t)i1; a.m = (uint32_t)t->m;
+    a.xa = xa; a.xb = xb; a.xw = xw; a.xm = xm;
     a.ta = t->ta[cur]; a.tb = t->tb[cur]; a.tw = t->tw[cur];
     a.na = t->ta[nxt]; a.nb = t->tb[nxt]; a.nw = t->tw[nxt];
     a.parent = t->parent;
     a.cw_row = t->cand_w[0]; a.co_row = t->cand_o[0]; a.cw_col = t->cand_w[1]; a.co_col = t->cand_o[1];
     a.best_w = t->best_w; a.best_id = t->best_id; a.counters = t->counters;
+    const bool dense = i1 > i0 && i1 >= 2;
     const int64_t out_base = i0 * (i0 - 1) / 2;
     const unsigned gv = (unsigned)((a.n + 255) / 256);
-    const unsigned gi = (unsigned)((2ull * a.n + a.m + 255) / 256);
+    const unsigned gi = (unsigned)((2ull * a.n + a.m + a.xm + 255) / 256);
+    // a dense row v links every u < v, so after any dense update leaves 0..max_row_end-1 are ONE component
+    // and the leaves above are singletons: the round that reaches that count is the last one.  Without a
+    // dense block (merge of sparse edges) the loop ends on the first round that hooks nothing.
+    const int64_t max_end = std::max<int64_t>(t->max_row_end, dense ? i1 : 0);
+    const uint32_t roots_done = max_end >= 2 ? (uint32_t)(1 + t->k - max_end) : (uint32_t)t->k;
     int cb = 0;                                            // which comp buffer holds the current labels
-    if (a.n >= 2) {
-        for (int round = 0; round < 64; ++round) {
-            a.comp = t->comp[cb]; a.comp_next = t->comp[cb ^ 1];
-            tree_reset_kernel<<<gv, 256, 0, st>>>(a, round == 0);
+    uint32_t hooked = 0;
+    for (int round = 0; round < 64; ++round) {
+        a.comp = t->comp[cb]; a.comp_next = t->comp[cb ^ 1];
+        tree_reset_kernel<<<gv, 256, 0, st>>>(a, round == 0);
+        if (dense) {
             tree_row_kernel<<<(unsigned)(i1 - i0), 256, 0, st>>>(sim_block, a.i0, a.i1, out_base, a.comp, t->cand_w[0], t->cand_o[0]);
             tree_col_kernel<<<(unsigned)((a.i1 - 1 + 255) / 256), 256, 0, st>>>(sim_block, a.i0, a.i1, out_base, a.comp, t->cand_w[1], t->cand_o[1]);
-            tree_best_kernel<0><<<gi, 256, 0, st>>>(a);
-            tree_best_kernel<1><<<gi, 256, 0, st>>>(a);
-            tree_hook_kernel<<<gv, 256, 0, st>>>(a);
-            tree_relabel_kernel<<<gv, 256, 0, st>>>(a);
-            FAMSA_CUDA(cudaMemcpyAsync(t->h_counters, t->counters, 2 * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
-            FAMSA_CUDA(cudaStreamSynchronize(st));
-            t->launches += 7; t->rounds++;
-            cb ^= 1;
-            if (t->h_counters[1] <= 1) break;
+            t->launches += 2;
         }
-        FAMSA_CUDA(cudaGetLastError());
-        if (t->h_counters[1] != 1 || t->h_counters[0] != a.n - 1) {
-            set_error("famsa_tree_update: Boruvka did not converge (NaN similarities?)"); return FAMSA_EINVAL;
-        }
+        tree_best_kernel<0><<<gi, 256, 0, st>>>(a);
+        tree_best_kernel<1><<<gi, 256, 0, st>>>(a);
+        tree_hook_kernel<<<gv, 256, 0, st>>>(a);
+        tree_relabel_kernel<<<gv, 256, 0, st>>>(a);
+        FAMSA_CUDA(cudaMemcpyAsync(t->h_counters, t->counters, 2 * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+        FAMSA_CUDA(cudaStreamSynchronize(st));
+        t->launches += 5; t->rounds++;
+        cb ^= 1;
+        const bool progress = t->h_counters[0] != hooked;
+        hooked = t->h_counters[0];
+        if (!progress || (!t->merged && xm == 0 && t->h_counters[1] == roots_done)) break;
     }
-    t->cur = nxt; t->rows = i1;
+    FAMSA_CUDA(cudaGetLastError());
+    if (hooked + t->h_counters[1] != (uint32_t)t->k || (!t->merged && xm == 0 && t->h_counters[1] != roots_done)) {
+        set_error("famsa_tree: Boruvka did not converge (NaN similarities?)"); return FAMSA_EINVAL;
+    }
+    t->cur = nxt; t->m = hooked; t->max_row_end = max_end;
     return FAMSA_OK;
 }
 
+}  // namespace famsa
+
+extern "C" int famsa_tree_update(famsa_tree* t, int64_t i0, int64_t i1, const float* sim_block, void* cuda_stream) {
+    if (!t) { set_error("famsa_tree_update: tree is NULL"); return FAMSA_EINVAL; }
+    if (i0 < 0 || i1 < i0 || i1 > t->k) { set_error("famsa_tree_update: bad row range"); return FAMSA_ERANGE; }
+    if (i1 == i0) return FAMSA_OK;
+    if (!sim_block && famsa_rows_pairs(i0, i1) > 0) { set_error("famsa_tree_update: sim_block is NULL"); return FAMSA_EINVAL; }
+    FAMSA_CUDA(cudaSetDevice(t->device));
+    if (famsa_rows_pairs(i0, i1) > 0) {
+        int rc = tree_rounds(t, i0, i1, sim_block, nullptr, nullptr, nullptr, 0, (cudaStream_t)cuda_stream);
+        if (rc != FAMSA_OK) return rc;
+    }
+    t->rows += i1 - i0;
+    return FAMSA_OK;
+}
+
+extern "C" int famsa_tree_merge_edges(famsa_tree* t, const int64_t* a_host, const int64_t* b_host, const float* sim_host, int64_t m) {
+    if (!t) { set_error("famsa_tree_merge_edges: tree is NULL"); return FAMSA_EINVAL; }
+    if (m < 0 || (m > 0 && (!a_host || !b_host || !sim_host))) { set_error("famsa_tree_merge_edges: null input"); return FAMSA_EINVAL; }
+    if (m == 0) return FAMSA_OK;
+    if (m > 0x7FFFFFF0LL) { set_error("famsa_tree_merge_edges: too many edges"); return FAMSA_EINVAL; }
+    FAMSA_CUDA(cudaSetDevice(t->device));
+    std::vector<uint32_t> a(m), b(m);
+    for (int64_t e = 0; e < m; ++e) {
+        if (a_host[e] < 0 || a_host[e] >= t->k || b_host[e] < 0 || b_host[e] >= t->k || !(sim_host[e] >= 0.0f)) {
+            set_error("famsa_tree_merge_edges: edge " + std::to_string(e) + " has a leaf out of range or a negative/NaN similarity");
+            return FAMSA_ERANGE;
+        }
+        a[e] = (uint32_t)a_host[e]; b[e] = (uint32_t)b_host[e];
+    }
+    uint32_t *xa = nullptr, *xb = nullptr; float* xw = nullptr;
+    cudaError_t e1 = cudaMalloc((void**)&xa, 4ull * m), e2 = cudaMalloc((void**)&xb, 4ull * m), e3 = cudaMalloc((void**)&xw, 4ull * m);
+    int rc = FAMSA_OK;
+    if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
+        cudaGetLastError(); set_error("famsa_tree_merge_edges: device allocation failed"); rc = FAMSA_ENOMEM;
+    } else if (cudaMemcpy(xa, a.data(), 4ull * m, cudaMemcpyHostToDevice) != cudaSuccess ||
+               cudaMemcpy(xb, b.data(), 4ull * m, cudaMemcpyHostToDevice) != cudaSuccess ||
+               cudaMemcpy(xw, sim_host, 4ull * m, cudaMemcpyHostToDevice) != cudaSuccess) {
+        rc = famsa::cuda_fail(cudaGetLastError(), "famsa_tree_merge_edges: copy");
+    } else {
+        rc = tree_rounds(t, 0, 0, nullptr, xa, xb, xw, (uint32_t)m, nullptr);
+        if (rc == FAMSA_OK) t->merged = true;
+    }
+    cudaFree(xa); cudaFree(xb); cudaFree(xw);
+    return rc;
+}
+
+extern "C" int64_t famsa_tree_edge_count(const famsa_tree* t) { return t ? t->m : 0; }
+
 extern "C" int famsa_tree_edges(famsa_tree* t, int64_t* a_host, int64_t* b_host, float* sim_host) {
     if (!t) { set_error("famsa_tree_edges: tree is NULL"); return FAMSA_EINVAL; }
-    const int64_t m = t->rows > 0 ? t->rows - 1 : 0;
+    const int64_t m = t->m;
     if (m == 0) return FAMSA_OK;
     if (!a_host || !b_host || !sim_host) { set_error("famsa_tree_edges: null output"); return FAMSA_EINVAL; }
     FAMSA_CUDA(cudaSetDevice(t->device));
@@ -343,8 +409,11 @@ __global__ void tree_dendrogram_kernel(uint32_t k, const uint32_t* order, const 
 
 extern "C" int famsa_tree_finish(famsa_tree* t, int64_t* id_a_host, int64_t* id_b_host, float* sim_host, int64_t* size_host) {
     if (!t) { set_error("famsa_tree_finish: tree is NULL"); return FAMSA_EINVAL; }
-    if (t->rows != t->k) { set_error("famsa_tree_finish: only " + std::to_string(t->rows) + " of " + std::to_string(t->k) + " rows consumed"); return FAMSA_ERANGE; }
     if (t->k < 2) return FAMSA_OK;
+    if (t->m != t->k - 1 || (!t->merged && t->rows < t->k)) {
+        set_error("famsa_tree_finish: the forest has " + std::to_string(t->m) + " of " + std::to_string(t->k - 1) +
+                  " edges: not every row has been consumed or merged in"); return FAMSA_ERANGE;
+    }
     if (!id_a_host || !id_b_host || !sim_host || !size_host) { set_error("famsa_tree_finish: null output"); return FAMSA_EINVAL; }
     FAMSA_CUDA(cudaSetDevice(t->device));
     const uint32_t k = (uint32_t)t->k, m = k - 1;
@@ -379,60 +448,77 @@ extern "C" int famsa_tree_finish(famsa_tree* t, int64_t* id_a_host, int64_t* id_
     return FAMSA_OK;
 }
 
-extern "C" int famsa_guide_tree(famsa_ctx* ctx, int64_t block_rows, int64_t* id_a_host, int64_t* id_b_host,
-                                float* sim_host, int64_t* size_host) {
-    if (!ctx) { set_error("famsa_guide_tree: ctx is NULL"); return FAMSA_EINVAL; }
-    if (block_rows < 0) { set_error("famsa_guide_tree: block_rows < 0"); return FAMSA_EINVAL; }
+extern "C" int famsa_guide_forest(famsa_ctx* ctx, int64_t block_rows, int64_t part, int64_t parts, famsa_tree** out) {
+    if (!out) { set_error("famsa_guide_forest: out is NULL"); return FAMSA_EINVAL; }
+    *out = nullptr;
+    if (!ctx) { set_error("famsa_guide_forest: ctx is NULL"); return FAMSA_EINVAL; }
+    if (block_rows < 0 || parts < 1 || part < 0 || part >= parts) { set_error("famsa_guide_forest: bad block_rows / part / parts"); return FAMSA_EINVAL; }
     if (block_rows == 0) block_rows = 1024;
     const int64_t k = ctx->k;
-    if (k < 2) return FAMSA_OK;
     FAMSA_CUDA(cudaSetDevice(ctx->device));
     famsa_tree* t = nullptr;
     int rc = famsa_tree_create(k, ctx->device, &t);
     if (rc != FAMSA_OK) return rc;
-    const int64_t nb = (k + block_rows - 1) / block_rows;
-    const int64_t max_pairs = famsa_rows_pairs(std::max<int64_t>(k - block_rows, 0), k);
+    const int64_t nb_all = (k + block_rows - 1) / block_rows;
+    std::vector<int64_t> mine;                             // this part's row blocks: part, part + parts, ...
+    for (int64_t b = part; b < nb_all; b += parts) mine.push_back(b);
+    const int64_t nb = (int64_t)mine.size();
+    if (k < 2 || nb == 0) { *out = t; return FAMSA_OK; }
+    auto rows_of = [&](int64_t n, int64_t& i0, int64_t& i1) { i0 = mine[n] * block_rows; i1 = std::min(i0 + block_rows, k); };
+    int64_t i0, i1;
+    int64_t max_pairs = 1;                                 // (the last block may be short: take the max)
+    for (int64_t n = 0; n < nb; ++n) { rows_of(n, i0, i1); max_pairs = std::max(max_pairs, famsa_rows_pairs(i0, i1)); }
     float* buf[2] = {nullptr, nullptr};
     cudaStream_t sa = nullptr, sb = nullptr;
     cudaEvent_t ev[2] = {nullptr, nullptr};
-    auto cleanup = [&]() {
+    auto cleanup = [&](bool keep_tree) {
         cudaDeviceSynchronize();
         cudaFree(buf[0]); cudaFree(buf[1]);
         if (sa) cudaStreamDestroy(sa);
         if (sb) cudaStreamDestroy(sb);
         if (ev[0]) cudaEventDestroy(ev[0]);
         if (ev[1]) cudaEventDestroy(ev[1]);
-        famsa_tree_free(t);
+        if (!keep_tree) famsa_tree_free(t);
     };
 #define GT_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { int r__ = (e__ == cudaErrorMemoryAllocation) ? FAMSA_ENOMEM : FAMSA_ECUDA; \
-        famsa::cuda_fail(e__, #call); cleanup(); return r__; } } while (0)
-#define GT_TRY(x) do { int r__ = (x); if (r__ != FAMSA_OK) { cleanup(); return r__; } } while (0)
+        famsa::cuda_fail(e__, #call); cleanup(false); return r__; } } while (0)
+#define GT_TRY(x) do { int r__ = (x); if (r__ != FAMSA_OK) { cleanup(false); return r__; } } while (0)
     GT_CUDA(cudaMalloc((void**)&buf[0], std::max<int64_t>(max_pairs, 1) * sizeof(float)));
     GT_CUDA(cudaMalloc((void**)&buf[1], std::max<int64_t>(max_pairs, 1) * sizeof(float)));
     GT_CUDA(cudaStreamCreateWithFlags(&sa, cudaStreamNonBlocking));
     GT_CUDA(cudaStreamCreateWithFlags(&sb, cudaStreamNonBlocking));
     GT_CUDA(cudaEventCreateWithFlags(&ev[0], cudaEventDisableTiming));
     GT_CUDA(cudaEventCreateWithFlags(&ev[1], cudaEventDisableTiming));
-    auto rows_of = [&](int64_t b, int64_t& i0, int64_t& i1) { i0 = b * block_rows; i1 = std::min(i0 + block_rows, k); };
-    int64_t i0, i1;
     rows_of(0, i0, i1);
     if (famsa_rows_pairs(i0, i1) > 0) GT_TRY(famsa::sweep_rows(ctx, i0, i1, nullptr, buf[0], sa));
     GT_CUDA(cudaEventRecord(ev[0], sa));
-    for (int64_t b = 0; b < nb; ++b) {
-        if (b + 1 < nb) {                                  // sweep the next block while this one is merged
+    for (int64_t n = 0; n < nb; ++n) {
+        if (n + 1 < nb) {                                  // sweep the next block while this one is merged
             int64_t n0, n1;
-            rows_of(b + 1, n0, n1);
-            GT_TRY(famsa::sweep_rows(ctx, n0, n1, nullptr, buf[(b + 1) & 1], sa));
-            GT_CUDA(cudaEventRecord(ev[(b + 1) & 1], sa));
+            rows_of(n + 1, n0, n1);
+            GT_TRY(famsa::sweep_rows(ctx, n0, n1, nullptr, buf[(n + 1) & 1], sa));
+            GT_CUDA(cudaEventRecord(ev[(n + 1) & 1], sa));
         }
-        rows_of(b, i0, i1);
-        GT_CUDA(cudaStreamWaitEvent(sb, ev[b & 1], 0));
-        GT_TRY(famsa_tree_update(t, i0, i1, buf[b & 1], sb));
+        rows_of(n, i0, i1);
+        GT_CUDA(cudaStreamWaitEvent(sb, ev[n & 1], 0));
+        GT_TRY(famsa_tree_update(t, i0, i1, buf[n & 1], sb));
     }
-    rc = famsa_tree_finish(t, id_a_host, id_b_host, sim_host, size_host);
     ctx->launches += t->launches;
-    cleanup();
-    return rc;
+    cleanup(true);
+    *out = t;
+    return FAMSA_OK;
 #undef GT_CUDA
 #undef GT_TRY
+}
+
+extern "C" int famsa_guide_tree(famsa_ctx* ctx, int64_t block_rows, int64_t* id_a_host, int64_t* id_b_host,
+                                float* sim_host, int64_t* size_host) {
+    famsa_tree* t = nullptr;
+    int rc = famsa_guide_forest(ctx, block_rows, 0, 1, &t);
+    if (rc != FAMSA_OK) return rc;
+    const int64_t before = t->launches;
+    rc = famsa_tree_finish(t, id_a_host, id_b_host, sim_host, size_host);
+    ctx->launches += t->launches - before;
+    famsa_tree_free(t);
+    return rc;
 }

@@ -18,8 +18,9 @@ FAMSA_MAX_LEN = 65535
 EXPORTS = ["famsa_pack", "famsa_lcs_rows", "famsa_lcs_rows_host", "famsa_rows_pairs", "famsa_rows_cells",
            "famsa_k", "famsa_perm", "famsa_lengths", "famsa_codes", "famsa_match", "famsa_launch_count",
            "famsa_alu_peak", "famsa_set_tuning", "famsa_free", "famsa_strerror", "famsa_last_error",
-           "famsa_tree_create", "famsa_tree_update", "famsa_tree_edges", "famsa_tree_finish", "famsa_tree_free",
-           "famsa_guide_tree"]
+           "famsa_tree_create", "famsa_tree_update", "famsa_tree_merge_edges", "famsa_tree_edge_count",
+           "famsa_tree_edges", "famsa_tree_finish", "famsa_tree_free",
+           "famsa_guide_tree", "famsa_guide_forest"]
 
 
 class FamsaError(RuntimeError):
@@ -72,12 +73,18 @@ def lib():
         L.famsa_tree_create.argtypes = [i64, i32, ctypes.POINTER(vp)]
         L.famsa_tree_update.restype = i32
         L.famsa_tree_update.argtypes = [vp, i64, i64, vp, vp]
+        L.famsa_tree_merge_edges.restype = i32
+        L.famsa_tree_merge_edges.argtypes = [vp, vp, vp, vp, i64]
+        L.famsa_tree_edge_count.restype = i64
+        L.famsa_tree_edge_count.argtypes = [vp]
         L.famsa_tree_edges.restype = i32
         L.famsa_tree_edges.argtypes = [vp, vp, vp, vp]
         L.famsa_tree_finish.restype = i32
         L.famsa_tree_finish.argtypes = [vp, vp, vp, vp, vp]
         L.famsa_tree_free.restype = None
         L.famsa_tree_free.argtypes = [vp]
+        L.famsa_guide_forest.restype = i32
+        L.famsa_guide_forest.argtypes = [vp, i64, i64, i64, ctypes.POINTER(vp)]
         L.famsa_guide_tree.restype = i32
         L.famsa_guide_tree.argtypes = [vp, i64, vp, vp, vp, vp]
         L.famsa_strerror.restype = ctypes.c_char_p
@@ -266,11 +273,24 @@ def famsa_tree_update(tree, i0, i1, sim_block, cuda_stream=None):
         assert sim_block.is_cuda and sim_block.is_contiguous() and sim_block.element_size() == 4
         assert sim_block.numel() >= famsa_rows_pairs(i0, i1)
     _check(lib().famsa_tree_update(tree.handle, int(i0), int(i1), _ptr(sim_block), cuda_stream))
-    tree.rows = int(i1)
+    tree.rows += int(i1) - int(i0)
+
+
+def famsa_tree_merge_edges(tree, a, b, sim):
+    """HOST arrays: leaves a[e], b[e] (int64) and similarities sim[e] (float32) of the edges to merge in."""
+    a = np.ascontiguousarray(a, dtype=np.int64)
+    b = np.ascontiguousarray(b, dtype=np.int64)
+    sim = np.ascontiguousarray(sim, dtype=np.float32)
+    assert a.size == b.size == sim.size
+    _check(lib().famsa_tree_merge_edges(tree.handle, a.ctypes.data, b.ctypes.data, sim.ctypes.data, a.size))
+
+
+def famsa_tree_edge_count(tree):
+    return int(lib().famsa_tree_edge_count(tree.handle))
 
 
 def famsa_tree_edges(tree):
-    m = max(tree.rows - 1, 0)
+    m = famsa_tree_edge_count(tree)
     a, b, w = np.empty(m, np.int64), np.empty(m, np.int64), np.empty(m, np.float32)
     _check(lib().famsa_tree_edges(tree.handle, a.ctypes.data, b.ctypes.data, w.ctypes.data))
     return a, b, w
@@ -288,3 +308,11 @@ def famsa_guide_tree(ctx, block_rows=0):
     a, b, w, s = np.empty(m, np.int64), np.empty(m, np.int64), np.empty(m, np.float32), np.empty(m, np.int64)
     _check(lib().famsa_guide_tree(ctx.handle, int(block_rows), a.ctypes.data, b.ctypes.data, w.ctypes.data, s.ctypes.data))
     return a, b, w, s
+
+
+def famsa_guide_forest(ctx, block_rows=0, part=0, parts=1):
+    """Stages I + II over row blocks part, part + parts, ...: returns the Tree (a forest unless parts == 1)."""
+    out = ctypes.c_void_p()
+    _check(lib().famsa_guide_forest(ctx.handle, int(block_rows), int(part), int(parts), ctypes.byref(out)))
+    t = Tree(out.value, famsa_k(ctx))
+    return t

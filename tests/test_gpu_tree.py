@@ -123,20 +123,75 @@ def test_guide_tree_end_to_end(F, oracle):
         assert size[-1] == k and np.all(np.diff(mw[~inf]) <= 0)
 
 
+def feed_blocks(F, tri, k, blocks):
+    import torch
+    t = F.famsa_tree_create(k)
+    for i0, i1 in blocks:
+        a, b = F.famsa_rows_pairs(0, i0), F.famsa_rows_pairs(0, i1)
+        blk = torch.from_numpy(tri[a:b].copy()).cuda() if b > a else torch.zeros(1, dtype=torch.float32, device="cuda")
+        F.famsa_tree_update(t, i0, i1, blk)
+    return t
+
+
+def test_any_order_and_rank_forests_merge(F):
+    """Row blocks in any order give the same tree weights; the forests of two 'ranks' that each consumed
+    every other block (the multi-GPU deal of bench.py), merged as edges, give the tree of the whole matrix."""
+    rng = np.random.default_rng(12)
+    k, block = 1500, 128
+    tri = (rng.integers(1, 3000, k * (k - 1) // 2) / 32.0).astype(np.float32)
+    ref = np.sort(kruskal_weights(tri, k))[::-1]
+    blocks = [(a, min(a + block, k)) for a in range(0, k, block)]
+    for order in (blocks[::-1], [blocks[i] for i in rng.permutation(len(blocks))]):
+        with feed_blocks(F, tri, k, order) as t:
+            a, b, w = F.famsa_tree_edges(t)
+            check_tree(a, b, w, tri, k)
+            assert np.array_equal(np.sort(w)[::-1], ref)
+    forests = []
+    for rank in range(2):
+        with feed_blocks(F, tri, k, blocks[rank::2]) as t:
+            assert F.famsa_tree_edge_count(t) <= k - 1
+            forests.append(F.famsa_tree_edges(t))
+            if rank == 1 and blocks[-1] not in blocks[rank::2]:
+                with pytest.raises(F.FamsaError):
+                    F.famsa_tree_finish(t)                       # this rank alone has not seen every row
+    with feed_blocks(F, tri, k, []) as t:
+        for a, b, w in forests:
+            F.famsa_tree_merge_edges(t, a, b, w)
+        a, b, w = F.famsa_tree_edges(t)
+        check_tree(a, b, w, tri, k)
+        assert np.array_equal(np.sort(w)[::-1], ref)
+        _, _, mw, size = F.famsa_tree_finish(t)
+        assert np.array_equal(mw, ref) and size[-1] == k
+    # merging edges into a tree that also consumes dense blocks afterwards
+    with feed_blocks(F, tri, k, []) as t:
+        F.famsa_tree_merge_edges(t, *forests[0])
+        for i0, i1 in blocks[1::2]:
+            a0, b0 = F.famsa_rows_pairs(0, i0), F.famsa_rows_pairs(0, i1)
+            import torch
+            F.famsa_tree_update(t, i0, i1, torch.from_numpy(tri[a0:b0].copy()).cuda())
+        _, _, w = F.famsa_tree_edges(t)
+        assert np.array_equal(np.sort(w)[::-1], ref)
+
+
 def test_tree_errors(F):
     import torch
     t = F.famsa_tree_create(5)
-    buf = torch.ones(10, dtype=torch.float32, device="cuda")
+    buf = torch.ones(32, dtype=torch.float32, device="cuda")
+    for i0, i1 in ((3, 2), (0, 6), (-1, 2)):
+        with pytest.raises(F.FamsaError) as e:
+            F.famsa_tree_update(t, i0, i1, buf)
+        assert e.value.code == F.FAMSA_ERANGE
+    F.famsa_tree_update(t, 3, 5, buf)                            # any order is legal ...
+    assert F.famsa_tree_edge_count(t) == 4
     with pytest.raises(F.FamsaError) as e:
-        F.famsa_tree_update(t, 1, 3, buf)                        # rows must arrive in order
+        F.famsa_tree_finish(t)                                   # ... but not every row has been consumed
     assert e.value.code == F.FAMSA_ERANGE
     F.famsa_tree_update(t, 0, 3, buf)
-    with pytest.raises(F.FamsaError) as e:
-        F.famsa_tree_finish(t)                                   # not all rows consumed
-    assert e.value.code == F.FAMSA_ERANGE
-    F.famsa_tree_update(t, 3, 5, buf)
     _, _, w, size = F.famsa_tree_finish(t)
     assert np.all(w == 1.0) and size[-1] == 5
+    with pytest.raises(F.FamsaError) as e:
+        F.famsa_tree_merge_edges(t, [7], [0], [1.0])             # leaf out of range
+    assert e.value.code == F.FAMSA_ERANGE
     t.free()
     for k in (0, 1):
         t = F.famsa_tree_create(k)
@@ -144,3 +199,20 @@ def test_tree_errors(F):
             F.famsa_tree_update(t, 0, 1, None)
         assert F.famsa_tree_finish(t)[0].size == 0
         t.free()
+
+
+def test_guide_forest_parts_merge_to_the_guide_tree(F):
+    """The multi-GPU deal on one device: forests of parts 0/3, 1/3, 2/3 of the row blocks, merged, equal
+    the single-pass guide tree (sorted merge similarities; sizes)."""
+    from paper_1603_06958_b200 import synth
+    seqs, offsets = synth.family(1, k=700, seed=33)
+    with F.famsa_pack(seqs, offsets) as ctx:
+        ia, ib, mw, size = F.famsa_guide_tree(ctx, 64)
+        forests = [F.famsa_guide_forest(ctx, 64, part, 3) for part in range(3)]
+        root = forests[0]
+        for other in forests[1:]:
+            F.famsa_tree_merge_edges(root, *F.famsa_tree_edges(other))
+        ia2, ib2, mw2, size2 = F.famsa_tree_finish(root)
+        for t in forests:
+            t.free()
+    assert np.array_equal(mw, mw2) and size2[-1] == 700 and np.array_equal(np.sort(size), np.sort(size2))

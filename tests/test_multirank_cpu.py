@@ -32,6 +32,43 @@ def _worker(rank, world, port, k, stride, out):
     dist.destroy_process_group()
 
 
+def _gather_worker(rank, world, port, out):
+    import torch
+    import torch.distributed as dist
+    import bench
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    k = 50
+    rng = np.random.default_rng(100 + rank)
+    m = 17 if rank == 0 else 49                                  # forests of different sizes, one of them full
+    a = rng.integers(1, k, m).astype(np.int64); b = (a * rng.random(m)).astype(np.int64); w = rng.random(m).astype(np.float32)
+    parts = bench.gather_forests(dist, a, b, w, k, torch.device("cpu"))
+    out.put((rank, [(x.tolist(), y.tolist(), z.tolist()) for x, y, z in parts], (a.tolist(), b.tolist(), w.tolist())))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_gather_forests_gloo():
+    """The one exchange step of the multi-GPU guide tree (bench.gather_forests): a padded all_gather."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 31500 + (os.getpid() % 2000)
+    procs = [ctx.Process(target=_gather_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    mine = {r: own for r, _, own in res}
+    for r, parts, _ in res:
+        assert len(parts) == 2
+        for src in range(2):
+            assert tuple(parts[src]) == tuple(mine[src])         # every rank holds every rank's edges, unpadded
+
+
 @pytest.mark.parametrize("stride", [2, 1])
 def test_two_ranks_gloo(stride):
     import torch.multiprocessing as mp
