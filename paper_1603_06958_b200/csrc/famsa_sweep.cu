@@ -2,13 +2,13 @@
 // similarity epilogue and packed-triangular row store (recurrence as
 // stated in BASELINE.json north_star, cited by the paper as Hyyro [15]).
 //
-// Mapping: one thread = one pair at a time.  A CTA owns TA rows (A side:
-// match tables staged in shared memory, layout [word][symbol] so one warp load = one 128-byte
-// row, no bank conflict for any residue mix) x TB columns (B side: thread t walks sequence
-// j0 + t; a warp = one 32-lane interleave group, so each uint4 load is 512 contiguous bytes).
-// V lives in W registers; the add carry runs through the hardware carry flag
-// (add.cc / addc.cc -> IADD3 / IADD3.X).  Per 32-bit word-step: LOP3, IADD3.X, LOP3 + one LDS.
-// Rows longer than 32 words are cut into blocks of Wb <= 32 words; the carry out of block t at
+// Mapping: one thread sweeps NR = 1-3 rows (A side) against one column (B side).
+// A CTA owns TA rows (their match tables arrive in shared memory by one TMA bulk copy; layout
+// [word][symbol], so one warp load = one 128-byte row and no residue mix can bank-conflict) x TB = 128
+// columns (thread t walks sequence j0 + t; a warp = one 32-lane interleave group, so each uint4 load
+// is 512 contiguous bytes).  V lives in NR x W registers; the add carry runs through the hardware
+// carry flag (add.cc / addc.cc -> IADD3 / IADD3.X).  Per 32-bit word-step: LOP3, IADD3.X, LOP3 + one
+// LDS.  Rows longer than 32 words are cut into blocks of Wb <= 32 words; the carry out of block t at
 // residue p is kept in a per-thread bit-vector and fed to block t+1 at residue p.
 #include <algorithm>
 

@@ -1,12 +1,13 @@
 // famsa_tree.cu -- stage II consumer: single-linkage guide tree built incrementally from the streamed
 // similarity row blocks in O(k) memory.  See include/famsa_lcs.h.
 //
-// State: the maximum spanning tree T of the complete similarity graph over the rows consumed so far
-// (n-1 edges).  Single linkage = T's edges taken by decreasing similarity, so T is an O(k) summary
-// from which the dendrogram follows, and MST(G + new rows) = MST(T + new rows): a row block [i0, i1)
-// is merged in by Boruvka rounds over the graph (T's edges) + (the block's dense entries (v, u < v)).
+// State: the maximum spanning FOREST T of the similarity entries seen so far (<= k-1 edges).  Single
+// linkage = the spanning tree's edges taken by decreasing similarity, so T is an O(k) summary from which
+// the dendrogram follows, and MSF(E1 u E2) = MSF(MSF(E1) u E2): a row block [i0, i1) -- in any order --
+// is merged in by Boruvka rounds over (T's edges) + (the block's dense entries (v, u < v)); the forests
+// of several ranks are merged the same way from their edge lists (famsa_tree_merge_edges).
 // Every edge has a unique key (similarity descending, then (max, min) endpoint ascending), so each
-// round's picks are edges of the one MST under that order and only mutual picks form 2-cycles.
+// round's picks are edges of the one MSF under that order and only mutual picks form 2-cycles.
 // A round is data-parallel: two streaming passes over the block (best edge per new row, best edge
 // per column), then O(k) per-component reductions with 32/64-bit atomics, hooking and relabelling.
 #include <cub/device/device_radix_sort.cuh>
