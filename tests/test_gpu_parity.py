@@ -273,3 +273,25 @@ def test_alu_peak_is_sane(F):
     assert 55.0 < p["instr_per_clk_sm"] <= 64.5
     assert 1000.0 < p["sm_mhz"] < 2300.0
     assert p["instr_per_s"] == pytest.approx(p["instr_per_clk_sm"] * p["sm_mhz"] * 1e6 * 148, rel=0.05)
+
+
+def test_gpu_matches_stored_oracle_digests(F):
+    """The CUDA path against digests the oracle wrote earlier (tests/golden/oracle_digests.txt): the
+    expected values do not come from this run, nor ever from the CUDA path."""
+    import hashlib
+    import os
+    from paper_1603_06958_b200 import synth
+    path = os.path.join(os.path.dirname(__file__), "golden", "oracle_digests.txt")
+    n = 0
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        config, k, seed, residues, sha, total, n_inf, _ = line.split()
+        seqs, offsets = synth.family(int(config), k=int(k), seed=None if seed == "default" else int(seed))
+        assert seqs.size == int(residues)
+        with F.famsa_pack(seqs, offsets) as ctx:
+            lcs, sim = gpu_rows(F, ctx, 0, int(k))
+        assert hashlib.sha256(np.ascontiguousarray(lcs, dtype="<i4").tobytes()).hexdigest() == sha
+        assert int(lcs.sum()) == int(total) and int(np.isinf(sim).sum()) == int(n_inf)
+        n += 1
+    assert n == 5

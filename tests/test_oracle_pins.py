@@ -208,3 +208,19 @@ def test_bitparallel_cpu_baseline_matches_dp(oracle):
     fast = oracle.bitpar_pairs(flat, offsets, pi, pj, n_threads=3)
     slow, _ = oracle.pairs(flat, offsets, pi, pj, want_sim=False, n_threads=3)
     assert np.array_equal(fast, slow)
+
+
+def test_oracle_digests_are_stable(oracle):
+    """The oracle + the seeded generator still reproduce the stored digests (tests/golden/oracle_digests.txt,
+    written by tests/golden/make_goldens.py from oracle/ only): guards against silent drift of either."""
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_goldens", os.path.join(GOLDEN, "make_goldens.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    stored = [l.strip() for l in open(os.path.join(GOLDEN, "oracle_digests.txt")) if l.strip() and not l.startswith("#")]
+    assert len(stored) == len(mg.CASES)
+    for case, line in zip(mg.CASES, stored):
+        got = mg.digest(*case).split()
+        want = line.split()
+        assert got[:7] == want[:7], case
+        assert float(got[7]) == pytest.approx(float(want[7]), rel=1e-12)
