@@ -79,3 +79,47 @@ def test_config4_full_size_sampled(F, oracle):
     assert k == 415519
     last = (k - 1) // BLOCK_ROWS
     assert check_blocks(F, oracle, seqs, offsets, [0, 1, 96, 240, last - 1, last], 6000) == 36000
+
+
+def test_config4_one_million_sampled_pairs_of_the_full_sweep(F, oracle):
+    """BASELINE.json configs[4]: "~8.6e10 pairs computed as streamed row blocks, oracle checked on 1e6 seeded
+    sampled pairs".  The WHOLE sweep runs in the bench configuration (1024-row blocks, LCS + similarity);
+    from every block the sampled entries are gathered on the device; all of them are then checked against
+    the oracle: 1e6 uniform pairs plus the strata of synth.sample_pairs (longest x longest, shortest,
+    block-boundary rows, lengths = 0, 1, 31 mod 32) and the planted duplicates."""
+    import torch
+    from paper_1603_06958_b200 import synth
+    seqs, offsets = synth.family(4)
+    k = len(offsets) - 1
+    perm_ref = oracle.sort_perm(offsets)
+    with F.famsa_pack(seqs, offsets) as ctx:
+        lens = F.famsa_lengths(ctx)
+        si, sj = synth.sample_pairs(k, 1_000_000, seed=20260406, lengths_sorted=lens, block_rows=BLOCK_ROWS)
+        assert si.size >= 1_000_000 and np.all(sj < si)
+        order = np.argsort(si, kind="stable")
+        si, sj = si[order], sj[order]
+        nblocks = (k + BLOCK_ROWS - 1) // BLOCK_ROWS
+        bounds = np.searchsorted(si, np.arange(nblocks + 1) * BLOCK_ROWS)
+        max_pairs = F.famsa_rows_pairs(k - BLOCK_ROWS, k)
+        lcs = torch.empty(max_pairs, dtype=torch.uint16, device="cuda")
+        sim = torch.empty(max_pairs, dtype=torch.float32, device="cuda")
+        got_l = torch.empty(si.size, dtype=torch.int16, device="cuda")
+        got_s = torch.empty(si.size, dtype=torch.float32, device="cuda")
+        pos_all = torch.from_numpy(si * (si - 1) // 2 + sj).cuda()
+        for b in range(nblocks):
+            i0, i1 = b * BLOCK_ROWS, min((b + 1) * BLOCK_ROWS, k)
+            F.famsa_lcs_rows(ctx, i0, i1, lcs, sim)
+            lo, hi = int(bounds[b]), int(bounds[b + 1])
+            if hi > lo:
+                idx = pos_all[lo:hi] - i0 * (i0 - 1) // 2
+                got_l[lo:hi] = lcs.view(torch.int16)[idx]
+                got_s[lo:hi] = sim[idx]
+        torch.cuda.synchronize()
+        gl = got_l.cpu().numpy().view(np.uint16).astype(np.int64)
+        gs = got_s.cpu().numpy().astype(np.float64)
+    lref, sref = oracle.pairs(seqs, offsets, perm_ref[si], perm_ref[sj])
+    bad = np.flatnonzero(gl != lref)
+    assert bad.size == 0, (bad[:5], gl[bad[:5]], lref[bad[:5]])
+    fin = np.isfinite(sref)
+    assert np.array_equal(np.isinf(gs), ~fin) and (~fin).sum() >= 0
+    assert np.all(np.abs(gs[fin] - sref[fin]) <= 1e-6 * np.abs(sref[fin]))
