@@ -245,6 +245,17 @@ def test_random_sets(F, oracle):
         check_all_rows(F, oracle, seqs, offsets)
 
 
+def test_random_long_sets(F, oracle):
+    """Seeded random sets with sequences of up to 9 000 residues: the blocked path with 2-9 table blocks per row,
+    both carry-vector sizes (|B| <= 4096 and above), mixed with short rows in the same set."""
+    rng = np.random.default_rng(202)
+    for hi, k in ((4096, 14), (9000, 10), (2500, 24)):
+        lens = [int(x) for x in rng.integers(1025, hi + 1, k // 2)] + [int(x) for x in rng.integers(1, 1200, k - k // 2)]
+        seq_list = [rng.integers(0, int(rng.choice([4, 20])), n).astype(np.uint8) for n in lens]
+        seqs, offsets = make_set(seq_list)
+        check_all_rows(F, oracle, seqs, offsets)
+
+
 def test_two_streams_one_ctx(F, oracle):
     """One ctx serves concurrent famsa_lcs_rows calls on different streams (it is read-only after pack)."""
     import torch
