@@ -76,31 +76,45 @@ __global__ void __launch_bounds__(256) tree_row_kernel(const float* __restrict__
 }
 
 // Best edge of each vertex u < i1-1 (a column) to a different component, over the block's rows v > u.
-__global__ void __launch_bounds__(256) tree_col_kernel(const float* __restrict__ sim, uint32_t i0, uint32_t i1, int64_t out_base,
-                                                       const uint32_t* __restrict__ comp, float* __restrict__ cw, uint32_t* __restrict__ co) {
+// A CTA covers 64 consecutive columns with 8 row slices (threadIdx.y): consecutive threads read
+// consecutive floats of a row (coalesced), each thread keeps several independent loads in flight, and
+// the 8 slices of a column are combined in shared memory.  HBM-bound: one pass over the block.
+constexpr int COL_X = 64, COL_Y = 8;
+__global__ void __launch_bounds__(COL_X * COL_Y) tree_col_kernel(const float* __restrict__ sim, uint32_t i0, uint32_t i1, int64_t out_base,
+                                                                 const uint32_t* __restrict__ comp, float* __restrict__ cw, uint32_t* __restrict__ co) {
     __shared__ uint32_t scomp[1024];
-    const uint32_t u = blockIdx.x * 256 + threadIdx.x;
+    __shared__ float sw[COL_Y][COL_X];
+    __shared__ uint32_t so[COL_Y][COL_X];
+    const uint32_t tid = threadIdx.y * COL_X + threadIdx.x;
+    const uint32_t u = blockIdx.x * COL_X + threadIdx.x;
     const bool live = u + 1 < i1;
     const uint32_t cu = live ? comp[u] : 0;
     float bw = NO_EDGE; uint32_t bo = 0xFFFFFFFFu;
     for (uint32_t t0 = i0; t0 < i1; t0 += 1024) {           // the block's rows, 1024 at a time
         const uint32_t t1 = min(t0 + 1024, i1);
         __syncthreads();
-        for (uint32_t t = threadIdx.x; t0 + t < t1; t += 256) scomp[t] = comp[t0 + t];
+        for (uint32_t t = tid; t0 + t < t1; t += COL_X * COL_Y) scomp[t] = comp[t0 + t];
         __syncthreads();
         if (live) {
-            uint32_t v = max(t0, u + 1);
-            int64_t off = (int64_t)v * (v - 1) / 2 - out_base + u;
-            for (; v < t1; ++v) {
+            // rows v = first + threadIdx.y, + COL_Y, ...  (first = the first row of this pass below column u)
+            const uint32_t first = max(t0, u + 1);
+#pragma unroll 4
+            for (uint32_t v = first + threadIdx.y; v < t1; v += COL_Y) {
                 if (scomp[v - t0] != cu) {
-                    const float w = __ldg(sim + off);
-                    if (w > bw) { bw = w; bo = v; }          // v ascends: the first of equal weights stays
+                    const float w = __ldg(sim + ((int64_t)v * (v - 1) / 2 - out_base + u));
+                    if (w > bw) { bw = w; bo = v; }          // v ascends within a slice: the first of equal weights stays
                 }
-                off += v;
             }
         }
     }
-    if (live) { cw[u] = bw; co[u] = bo; }
+    sw[threadIdx.y][threadIdx.x] = bw; so[threadIdx.y][threadIdx.x] = bo;
+    __syncthreads();
+    if (threadIdx.y == 0 && live) {
+#pragma unroll
+        for (int q = 1; q < COL_Y; ++q)
+            if (better(sw[q][threadIdx.x], so[q][threadIdx.x], bw, bo)) { bw = sw[q][threadIdx.x]; bo = so[q][threadIdx.x]; }
+        cw[u] = bw; co[u] = bo;
+    }
 }
 
 }  // namespace famsa
@@ -285,7 +299,7 @@ static int tree_rounds(famsa_tree* t, int64_t i0, int64_t i1, const float* sim_b
         tree_reset_kernel<<<gv, 256, 0, st>>>(a, round == 0);
         if (dense) {
             tree_row_kernel<<<(unsigned)(i1 - i0), 256, 0, st>>>(sim_block, a.i0, a.i1, out_base, a.comp, t->cand_w[0], t->cand_o[0]);
-            tree_col_kernel<<<(unsigned)((a.i1 - 1 + 255) / 256), 256, 0, st>>>(sim_block, a.i0, a.i1, out_base, a.comp, t->cand_w[1], t->cand_o[1]);
+            tree_col_kernel<<<(unsigned)((a.i1 - 1 + COL_X - 1) / COL_X), dim3(COL_X, COL_Y), 0, st>>>(sim_block, a.i0, a.i1, out_base, a.comp, t->cand_w[1], t->cand_o[1]);
             t->launches += 2;
         }
         tree_best_kernel<0><<<gi, 256, 0, st>>>(a);
