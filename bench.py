@@ -289,14 +289,17 @@ def run_cuda(args, rank, world, local_rank):
     e2e_pairs = pairs_step if one_call else max_pairs
     h_lcs = torch.empty(e2e_pairs, dtype=torch.uint16).pin_memory()
     h_sim = torch.empty(e2e_pairs, dtype=torch.float32).pin_memory() if want_sim else None
+    h_lcs2 = [h_lcs, h_lcs if one_call else torch.empty(e2e_pairs, dtype=torch.uint16).pin_memory()]
+    h_sim2 = [h_sim, h_sim if (one_call or not want_sim) else torch.empty(e2e_pairs, dtype=torch.float32).pin_memory()]
     e2e_steps = max(1, min(args.steps, 2))
     def e2e_step():
         c2 = F.famsa_pack(seqs, offsets, device=local_rank)
         if one_call:
             F.famsa_lcs_rows_host(c2, 0, k, h_lcs, h_sim)
         else:
-            for a, b in blocks:
-                F.famsa_lcs_rows_host(c2, a, b, h_lcs, h_sim)
+            for n, (a, b) in enumerate(blocks):               # two pinned row-block buffers, copies overlap the next sweep
+                F.famsa_lcs_rows_host_async(c2, a, b, h_lcs2[n & 1], h_sim2[n & 1] if want_sim else None)
+            F.famsa_sync(c2)
         c2.free()
     e2e_step()                                                # warm-up (allocations, staging buffers)
     barrier()

@@ -88,6 +88,19 @@ int famsa_lcs_rows(famsa_ctx* ctx, int64_t i0, int64_t i1,
 int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1,
                         uint16_t* lcs_host, float* sim_host);
 
+/*
+ * famsa_lcs_rows_host_async -- as above but returns once the work is ENQUEUED on the ctx's own streams, so
+ * the sweep of the next row block overlaps the device->host copy of this one (a streaming consumer calls it
+ * block after block with two host buffers).  The host buffers must be pinned for the copies to be
+ * asynchronous, must stay valid, and hold the results only after famsa_sync(ctx).  Calls of one ctx are
+ * ordered; do not mix concurrent host-path calls of one ctx from several threads.
+ */
+int famsa_lcs_rows_host_async(famsa_ctx* ctx, int64_t i0, int64_t i1,
+                              uint16_t* lcs_host, float* sim_host);
+
+/* Wait for everything the host path of this ctx has enqueued. */
+int famsa_sync(famsa_ctx* ctx);
+
 /* Number of (i, j < i) entries of rows [i0, i1): i1(i1-1)/2 - i0(i0-1)/2.  -1 if i0 > i1 or i0 < 0. */
 int64_t famsa_rows_pairs(int64_t i0, int64_t i1);
 

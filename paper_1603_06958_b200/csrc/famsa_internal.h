@@ -70,6 +70,7 @@ struct famsa_ctx {
     uint16_t* d_lcs_buf[2] = {nullptr, nullptr};
     float*    d_sim_buf[2] = {nullptr, nullptr};
     size_t    buf_pairs = 0;
+    int64_t   host_chunks = 0;                  // chunks enqueued by the host path so far
     cudaStream_t s_compute = nullptr, s_copy = nullptr;
     cudaEvent_t  ev_done[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
     std::atomic<int64_t> launches{0};

@@ -406,7 +406,7 @@ extern "C" int famsa_lcs_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* 
     return sweep_rows(ctx, i0, i1, lcs_out, sim_out, (cudaStream_t)cuda_stream);
 }
 
-extern "C" int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_host, float* sim_host) {
+static int rows_host_impl(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_host, float* sim_host, bool wait) {
     if (!ctx) { set_error("famsa_lcs_rows_host: ctx is NULL"); return FAMSA_EINVAL; }
     if (i0 < 0 || i0 > i1 || i1 > ctx->k) { set_error("famsa_lcs_rows_host: bad row range"); return FAMSA_ERANGE; }
     if (!lcs_host && !sim_host) { set_error("famsa_lcs_rows_host: both outputs are NULL"); return FAMSA_EINVAL; }
@@ -414,9 +414,9 @@ extern "C" int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1, uint1
     FAMSA_CUDA(cudaSetDevice(ctx->device));
     // lazily create the ping-pong staging (two row-block buffers of up to 32 Mi pairs each)
     // chunk size: about 1/8 of the call (so the copy of chunk n overlaps the sweep of chunk n+1),
-    // between 1 Mi and 32 Mi pairs, and never smaller than the longest row
+    // between 1 Mi and 128 Mi pairs, and never smaller than the longest row
     const int64_t total_pairs = famsa_rows_pairs(i0, i1);
-    const int64_t chunk_pairs = std::max<int64_t>(std::min<int64_t>(std::max<int64_t>(total_pairs / 8, (int64_t)1 << 20), (int64_t)32 << 20), i1);
+    const int64_t chunk_pairs = std::max<int64_t>(std::min<int64_t>(std::max<int64_t>(total_pairs / 8, (int64_t)1 << 20), (int64_t)128 << 20), i1);
     const size_t want = (size_t)std::min<int64_t>(total_pairs, chunk_pairs);
     if (!ctx->s_compute) {
         FAMSA_CUDA(cudaStreamCreateWithFlags(&ctx->s_compute, cudaStreamNonBlocking));
@@ -427,10 +427,10 @@ extern "C" int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1, uint1
         }
     }
     if (ctx->buf_pairs < want) {
-        // size the staging once per ctx (1/8 of the whole triangle, 1 Mi .. 32 Mi pairs, at least one row),
+        // size the staging once per ctx (1/8 of the whole triangle, 1 Mi .. 128 Mi pairs, at least one row),
         // so that a stream of growing row-block calls does not reallocate it
         const int64_t tri = ctx->k * (ctx->k - 1) / 2;
-        const size_t cap = (size_t)std::max<int64_t>(std::max<int64_t>(std::min<int64_t>(std::max<int64_t>(tri / 8, (int64_t)1 << 20), (int64_t)32 << 20), ctx->k), (int64_t)want);
+        const size_t cap = (size_t)std::max<int64_t>(std::max<int64_t>(std::min<int64_t>(std::max<int64_t>(tri / 8, (int64_t)1 << 20), (int64_t)128 << 20), ctx->k), (int64_t)want);
         FAMSA_CUDA(cudaDeviceSynchronize());
         for (int b = 0; b < 2; ++b) {
             cudaFree(ctx->d_lcs_buf[b]); cudaFree(ctx->d_sim_buf[b]);
@@ -447,13 +447,14 @@ extern "C" int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1, uint1
         ctx->buf_pairs = cap;
     }
     // chunk the row range so that each chunk fits a buffer (a single row always fits: i < 2^32 / ... k <= buf)
-    int64_t r = i0; int n = 0; int64_t done_pairs = 0;
+    int64_t r = i0; int64_t done_pairs = 0;
+    int64_t& n = ctx->host_chunks;                         // chunks enqueued so far by this ctx: the ping-pong continues across calls
     while (r < i1) {
         int64_t e = r + 1;
         while (e < i1 && famsa_rows_pairs(r, e + 1) <= (int64_t)want) ++e;
         const int64_t np = famsa_rows_pairs(r, e);
         if (np > (int64_t)ctx->buf_pairs) { set_error("famsa_lcs_rows_host: a single row exceeds the staging buffer"); return FAMSA_ENOMEM; }
-        const int b = n & 1;
+        const int b = (int)(n & 1);
         if (n >= 2) FAMSA_CUDA(cudaStreamWaitEvent(ctx->s_compute, ctx->ev_copied[b], 0));
         int rc = sweep_rows(ctx, r, e, lcs_host ? ctx->d_lcs_buf[b] : nullptr, sim_host ? ctx->d_sim_buf[b] : nullptr, ctx->s_compute);
         if (rc != FAMSA_OK) return rc;
@@ -464,7 +465,25 @@ extern "C" int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1, uint1
         FAMSA_CUDA(cudaEventRecord(ctx->ev_copied[b], ctx->s_copy));
         done_pairs += np; r = e; ++n;
     }
-    FAMSA_CUDA(cudaStreamSynchronize(ctx->s_copy));
-    FAMSA_CUDA(cudaStreamSynchronize(ctx->s_compute));
+    if (wait) {
+        FAMSA_CUDA(cudaStreamSynchronize(ctx->s_copy));
+        FAMSA_CUDA(cudaStreamSynchronize(ctx->s_compute));
+    }
+    return FAMSA_OK;
+}
+
+extern "C" int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_host, float* sim_host) {
+    return rows_host_impl(ctx, i0, i1, lcs_host, sim_host, true);
+}
+
+extern "C" int famsa_lcs_rows_host_async(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_host, float* sim_host) {
+    return rows_host_impl(ctx, i0, i1, lcs_host, sim_host, false);
+}
+
+extern "C" int famsa_sync(famsa_ctx* ctx) {
+    if (!ctx) { set_error("famsa_sync: ctx is NULL"); return FAMSA_EINVAL; }
+    FAMSA_CUDA(cudaSetDevice(ctx->device));
+    if (ctx->s_copy) FAMSA_CUDA(cudaStreamSynchronize(ctx->s_copy));
+    if (ctx->s_compute) FAMSA_CUDA(cudaStreamSynchronize(ctx->s_compute));
     return FAMSA_OK;
 }

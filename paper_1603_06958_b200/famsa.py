@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libfamsa_lcs.so")
 FAMSA_OK, FAMSA_EINVAL, FAMSA_ESYMBOL, FAMSA_ELENGTH, FAMSA_ERANGE, FAMSA_ENOMEM, FAMSA_ECUDA = 0, -1, -2, -3, -4, -5, -6
 FAMSA_MAX_LEN = 65535
 
-EXPORTS = ["famsa_pack", "famsa_lcs_rows", "famsa_lcs_rows_host", "famsa_rows_pairs", "famsa_rows_cells",
+EXPORTS = ["famsa_pack", "famsa_lcs_rows", "famsa_lcs_rows_host", "famsa_lcs_rows_host_async", "famsa_sync", "famsa_rows_pairs", "famsa_rows_cells",
            "famsa_k", "famsa_perm", "famsa_lengths", "famsa_codes", "famsa_match", "famsa_launch_count",
            "famsa_alu_peak", "famsa_set_tuning", "famsa_free", "famsa_strerror", "famsa_last_error",
            "famsa_tree_create", "famsa_tree_update", "famsa_tree_merge_edges", "famsa_tree_edge_count",
@@ -47,6 +47,10 @@ def lib():
         L.famsa_lcs_rows.argtypes = [vp, i64, i64, vp, vp, vp]
         L.famsa_lcs_rows_host.restype = i32
         L.famsa_lcs_rows_host.argtypes = [vp, i64, i64, vp, vp]
+        L.famsa_lcs_rows_host_async.restype = i32
+        L.famsa_lcs_rows_host_async.argtypes = [vp, i64, i64, vp, vp]
+        L.famsa_sync.restype = i32
+        L.famsa_sync.argtypes = [vp]
         L.famsa_rows_pairs.restype = i64
         L.famsa_rows_pairs.argtypes = [i64, i64]
         L.famsa_rows_cells.restype = i32
@@ -178,6 +182,20 @@ def famsa_lcs_rows_host(ctx, i0, i1, lcs_host, sim_host):
             else:
                 assert (not t.is_cuda) and t.is_contiguous() and t.element_size() == size and t.numel() >= n
     _check(lib().famsa_lcs_rows_host(ctx.handle, int(i0), int(i1), _ptr(lcs_host), _ptr(sim_host)))
+
+
+def famsa_lcs_rows_host_async(ctx, i0, i1, lcs_host, sim_host):
+    """As famsa_lcs_rows_host, but only enqueues (pinned CPU torch tensors / numpy views of pinned memory);
+    results are in the buffers after famsa_sync(ctx)."""
+    n = famsa_rows_pairs(i0, i1)
+    for t, size in ((lcs_host, 2), (sim_host, 4)):
+        if t is not None and not isinstance(t, np.ndarray):
+            assert (not t.is_cuda) and t.is_contiguous() and t.element_size() == size and t.numel() >= n
+    _check(lib().famsa_lcs_rows_host_async(ctx.handle, int(i0), int(i1), _ptr(lcs_host), _ptr(sim_host)))
+
+
+def famsa_sync(ctx):
+    _check(lib().famsa_sync(ctx.handle))
 
 
 def famsa_rows_cells(ctx, i0, i1):

@@ -306,3 +306,31 @@ def test_gpu_matches_stored_oracle_digests(F):
         assert int(lcs.sum()) == int(total) and int(np.isinf(sim).sum()) == int(n_inf)
         n += 1
     assert n == 5
+
+
+def test_host_path_async(F, oracle):
+    """famsa_lcs_rows_host_async + famsa_sync: row blocks streamed into two pinned host buffers give the
+    same values as the synchronous host call."""
+    import torch
+    from paper_1603_06958_b200 import synth
+    seqs, offsets = synth.family(1, k=1100, seed=61)
+    k, block = 1100, 256
+    with F.famsa_pack(seqs, offsets) as ctx:
+        n_all = F.famsa_rows_pairs(0, k)
+        ref_l = np.empty(n_all, np.uint16); ref_s = np.empty(n_all, np.float32)
+        F.famsa_lcs_rows_host(ctx, 0, k, ref_l, ref_s)
+        mp = F.famsa_rows_pairs(k - block, k)
+        hl = [torch.empty(mp, dtype=torch.uint16).pin_memory() for _ in range(2)]
+        hs = [torch.empty(mp, dtype=torch.float32).pin_memory() for _ in range(2)]
+        blocks = [(a, min(a + block, k)) for a in range(0, k, block)]
+        for n in range(0, len(blocks), 2):
+            pair = blocks[n:n + 2]
+            for q, (a, b) in enumerate(pair):
+                F.famsa_lcs_rows_host_async(ctx, a, b, hl[q], hs[q])
+            F.famsa_sync(ctx)
+            for q, (a, b) in enumerate(pair):
+                lo, hi = F.famsa_rows_pairs(0, a), F.famsa_rows_pairs(0, b)
+                assert np.array_equal(hl[q].numpy()[:hi - lo].view(np.uint16), ref_l[lo:hi])
+                assert np.array_equal(hs[q].numpy()[:hi - lo], ref_s[lo:hi])
+    lref, sref = oracle.rows(seqs, offsets, 0, k)
+    assert_match(ref_l.astype(np.int64), ref_s, lref, sref)
