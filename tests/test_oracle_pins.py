@@ -224,3 +224,33 @@ def test_oracle_digests_are_stable(oracle):
         want = line.split()
         assert got[:7] == want[:7], case
         assert float(got[7]) == pytest.approx(float(want[7]), rel=1e-12)
+
+
+def test_indel_is_a_metric(oracle):
+    """indel(A,B) = |A| + |B| - 2 LCS is the insertion/deletion edit distance, hence a metric:
+    zero iff equal, symmetric, triangle inequality.  A wrong LCS (too long or too short) breaks one of them."""
+    rng = np.random.default_rng(47)
+    for _ in range(120):
+        sigma = int(rng.choice([2, 3, 20]))
+        a, b, c = (rand_seq(rng, int(rng.integers(1, 80)), sigma) for _ in range(3))
+        d = lambda x, y: oracle.indel(len(x), len(y), oracle.lcs_len(x, y))
+        assert d(a, a) == 0 and (d(a, b) == 0) == (a == b)
+        assert d(a, b) == d(b, a)
+        assert d(a, c) <= d(a, b) + d(b, c)
+        assert (d(a, b) - (len(a) + len(b))) % 2 == 0 and abs(len(a) - len(b)) <= d(a, b) <= len(a) + len(b)
+
+
+def test_lcs_of_concatenations(oracle):
+    """LCS(A1+A2, B1+B2) >= LCS(A1,B1) + LCS(A2,B2) (superadditivity), with equality when the halves use
+    disjoint alphabets; and LCS(A+X, B+X) = LCS(A,B) + |X| for a common suffix X."""
+    rng = np.random.default_rng(53)
+    for _ in range(60):
+        a1, b1 = rand_seq(rng, int(rng.integers(1, 60)), 4), rand_seq(rng, int(rng.integers(1, 60)), 4)      # ACDE
+        a2 = "".join("FGHI"[i] for i in rng.integers(0, 4, int(rng.integers(1, 60))))
+        b2 = "".join("FGHI"[i] for i in rng.integers(0, 4, int(rng.integers(1, 60))))
+        l1, l2 = oracle.lcs_len(a1, b1), oracle.lcs_len(a2, b2)
+        assert oracle.lcs_len(a1 + a2, b1 + b2) == l1 + l2                                              # disjoint halves
+        m1, m2 = rand_seq(rng, 30, 4), rand_seq(rng, 30, 4)
+        assert oracle.lcs_len(a1 + m1, b1 + m2) >= l1 + oracle.lcs_len(m1, m2)
+        x = rand_seq(rng, int(rng.integers(1, 40)), 20)
+        assert oracle.lcs_len(a1 + x, b1 + x) == l1 + len(x)
