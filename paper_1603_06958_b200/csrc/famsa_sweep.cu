@@ -16,7 +16,10 @@
 
 namespace famsa {
 
-constexpr int TB = 128;          // threads (= columns) per CTA
+#ifndef FAMSA_TB
+#define FAMSA_TB 128
+#endif
+constexpr int TB = FAMSA_TB;     // threads (= columns) per CTA
 constexpr int MAX_ROWS_PER_LAUNCH = 1024;
 
 struct SweepArgs {
