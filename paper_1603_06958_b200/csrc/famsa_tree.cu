@@ -400,23 +400,44 @@ __global__ void tree_wkeys_kernel(uint32_t m, const float* tw, const uint32_t* i
     if (e < m) w_key[e] = ~__float_as_uint(tw[idx[e]]);     // ascending key == descending similarity
 }
 
-// The dendrogram from the sorted tree edges: a union-find pass, inherently sequential (one thread;
-// O(k alpha(k)) L2-resident steps, once per tree).
-__global__ void tree_dendrogram_kernel(uint32_t k, const uint32_t* order, const uint32_t* ta, const uint32_t* tb, const float* tw,
-                                       uint32_t* uf, long long* cid, long long* csize,
-                                       long long* out_a, long long* out_b, float* out_w, long long* out_size) {
-    if (blockIdx.x != 0 || threadIdx.x != 0) return;
-    for (uint32_t x = 0; x < k; ++x) { uf[x] = x; cid[x] = x; csize[x] = 1; }
-    for (uint32_t t = 0; t + 1 < k; ++t) {
-        const uint32_t e = order[t];
-        uint32_t ra = ta[e], rb = tb[e];
-        while (uf[ra] != ra) { uf[ra] = uf[uf[ra]]; ra = uf[ra]; }
-        while (uf[rb] != rb) { uf[rb] = uf[uf[rb]]; rb = uf[rb]; }
-        const long long ia = cid[ra], ib = cid[rb];
-        out_a[t] = ia < ib ? ia : ib; out_b[t] = ia < ib ? ib : ia; out_w[t] = tw[e];
-        if (csize[ra] < csize[rb]) { const uint32_t s = ra; ra = rb; rb = s; }
-        uf[rb] = ra; csize[ra] += csize[rb]; cid[ra] = (long long)k + t;
-        out_size[t] = csize[ra];
+// The dendrogram from the sorted tree edges: a union-find pass, inherently sequential (O(k alpha(k))
+// L2-resident steps, once per tree).  One warp: all lanes stage a batch of edges in shared memory and
+// write the batch's merges back (coalesced), lane 0 runs the union-find of the batch in between, so the
+// serial path touches global memory only for the union-find arrays themselves.
+constexpr int DG_BATCH = 1024;
+__global__ void __launch_bounds__(32) tree_dendrogram_kernel(uint32_t k, const uint32_t* order, const uint32_t* ta, const uint32_t* tb, const float* tw,
+                                                             uint32_t* uf, long long* cid, long long* csize,
+                                                             long long* out_a, long long* out_b, float* out_w, long long* out_size) {
+    __shared__ uint32_t sa[DG_BATCH], sb[DG_BATCH];
+    __shared__ long long oa[DG_BATCH], ob[DG_BATCH], os[DG_BATCH];
+    const uint32_t lane = threadIdx.x, m = k - 1;
+    for (uint32_t x = lane; x < k; x += 32) { uf[x] = x; cid[x] = x; csize[x] = 1; }
+    __syncwarp();
+    for (uint32_t t0 = 0; t0 < m; t0 += DG_BATCH) {
+        const uint32_t nb = min((uint32_t)DG_BATCH, m - t0);
+        for (uint32_t q = lane; q < nb; q += 32) {
+            const uint32_t e = order[t0 + q];
+            sa[q] = ta[e]; sb[q] = tb[e]; out_w[t0 + q] = tw[e];
+        }
+        __syncwarp();
+        if (lane == 0) {
+            for (uint32_t q = 0; q < nb; ++q) {
+                uint32_t ra = sa[q], rb = sb[q];
+                uint32_t pa = uf[ra], pb = uf[rb];                  // the two finds advance together
+                while (pa != ra || pb != rb) {
+                    if (pa != ra) { const uint32_t g = uf[pa]; uf[ra] = g; ra = g; pa = uf[ra]; }
+                    if (pb != rb) { const uint32_t g = uf[pb]; uf[rb] = g; rb = g; pb = uf[rb]; }
+                }
+                const long long ia = cid[ra], ib = cid[rb];
+                const long long za = csize[ra], zb = csize[rb];
+                oa[q] = ia < ib ? ia : ib; ob[q] = ia < ib ? ib : ia; os[q] = za + zb;
+                if (za < zb) { const uint32_t s = ra; ra = rb; rb = s; }
+                uf[rb] = ra; csize[ra] = za + zb; cid[ra] = (long long)k + t0 + q;
+            }
+        }
+        __syncwarp();
+        for (uint32_t q = lane; q < nb; q += 32) { out_a[t0 + q] = oa[q]; out_b[t0 + q] = ob[q]; out_size[t0 + q] = os[q]; }
+        __syncwarp();
     }
 }
 
