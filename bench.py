@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--stride", type=int, default=None, help="row-block stride of a step (default: 1 for configs 0-2, 16 for 3-4)")
     ap.add_argument("--full", action="store_true", help="a step is the full sweep whatever the config")
     ap.add_argument("--no-full", action="store_true", help="skip the extra single full sweep")
+    ap.add_argument("--strong", action="store_true",
+                    help="strong scaling: the N=1 batch of row blocks is dealt cyclically over the ranks (default: weak)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--guide-tree", action="store_true",
                     help="also time stages I+II (full sweep + single-linkage guide tree), the whole job dealt over the ranks")
@@ -174,11 +176,13 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
-def rank_blocks(k, stride, rank):
+def rank_blocks(k, stride, rank, world=1, strong=False):
     """The row blocks rank `rank` sweeps in one step.  Pairs are independent, so the path
     shards with no data-path collective: the packed set is replicated and row blocks are dealt by rank.
     stride > 1: rank r takes blocks r, r+stride, ... (disjoint batches of equal size: weak scaling);
     stride 1: the batch is the whole job and every rank sweeps its own replica of it."""
+    if strong:                                    # the N=1 batch, dealt block by block: block n of the batch -> rank n mod N
+        return step_blocks(k, stride)[rank::world]
     return step_blocks(k, stride, offset=rank if stride > 1 else 0)
 
 
@@ -236,7 +240,9 @@ def run_cuda(args, rank, world, local_rank):
     want_sim = args.config != 3                               # configs[3]: uint16 row blocks only
     stride = 1 if args.full else (args.stride or (1 if args.config <= 2 else 16))
     # weak scaling: rank r sweeps its own batch of row blocks (offset r), same size as the N=1 batch
-    blocks = rank_blocks(k, stride, rank)
+    blocks = rank_blocks(k, stride, rank, world, args.strong)
+    if not blocks:
+        blocks = step_blocks(k, stride)[:1]       # more ranks than blocks: repeat one block rather than idle (reported cells stay true)
 
     peak0 = F.famsa_alu_peak(local_rank)
     t0 = time.perf_counter()
@@ -421,7 +427,7 @@ def run_cuda(args, rank, world, local_rank):
         l2_note = "working set fits L2 (small config); ALU-bound path, no L2 flush between steps"
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong" if args.strong else "weak", "vs_baseline": None,
         "dtype": "u32", "data": "synthetic",
         "config": {"workload": WORKLOADS[args.config], "k": k,
                    "step": ("all rows" if stride == 1 else "every %d-th %d-row block (%d blocks)" % (stride, BLOCK_ROWS, len(blocks))),

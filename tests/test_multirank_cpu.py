@@ -105,3 +105,14 @@ def test_step_blocks_cover():
         rows = sorted(seen)
         assert rows[0][0] == 0 and rows[-1][1] == k and len(rows) == (k + 1023) // 1024
         assert all(rows[n][1] == rows[n + 1][0] for n in range(len(rows) - 1))
+
+
+def test_strong_scaling_deal():
+    """--strong: the N=1 batch is dealt block by block; the ranks' batches partition it."""
+    import bench
+    k, stride = 415519, 16
+    whole = bench.rank_blocks(k, stride, 0, 1, True)
+    assert whole == bench.step_blocks(k, stride)
+    parts = [bench.rank_blocks(k, stride, r, 4, True) for r in range(4)]
+    assert sorted(b for p in parts for b in p) == sorted(whole)
+    assert max(len(p) for p in parts) - min(len(p) for p in parts) <= 1
