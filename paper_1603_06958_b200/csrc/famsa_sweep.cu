@@ -415,7 +415,7 @@ static int rows_host_impl(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_
     if (!lcs_host && !sim_host) { set_error("famsa_lcs_rows_host: both outputs are NULL"); return FAMSA_EINVAL; }
     if (famsa_rows_pairs(i0, i1) == 0) return FAMSA_OK;
     FAMSA_CUDA(cudaSetDevice(ctx->device));
-    // lazily create the ping-pong staging (two row-block buffers of up to 32 Mi pairs each)
+    // lazily create the ping-pong staging (two staging buffers of 1 Mi .. 128 Mi pairs each)
     // chunk size: about 1/8 of the call (so the copy of chunk n overlaps the sweep of chunk n+1),
     // between 1 Mi and 128 Mi pairs, and never smaller than the longest row
     const int64_t total_pairs = famsa_rows_pairs(i0, i1);
