@@ -216,3 +216,31 @@ def test_guide_forest_parts_merge_to_the_guide_tree(F):
         for t in forests:
             t.free()
     assert np.array_equal(mw, mw2) and size2[-1] == 700 and np.array_equal(np.sort(size), np.sort(size2))
+
+
+def test_guide_tree_vs_scipy_at_k4000(F):
+    """Stages I + II on the device at k = 4000 against a library routine: scipy's single linkage run on the
+    rank-transformed similarities the device itself produced (so only stage II is under test here; stage I
+    has its own parity tests).  The merge similarities must agree exactly."""
+    from scipy.cluster.hierarchy import linkage
+    from paper_1603_06958_b200 import synth
+    import torch
+    k = 4000
+    seqs, offsets = synth.family(1, k=k, seed=71)
+    with F.famsa_pack(seqs, offsets) as ctx:
+        n = F.famsa_rows_pairs(0, k)
+        sim = torch.empty(n, dtype=torch.float32, device="cuda")
+        F.famsa_lcs_rows(ctx, 0, k, None, sim)
+        torch.cuda.synchronize()
+        tri = sim.cpu().numpy()
+        ia, ib, mw, size = F.famsa_guide_tree(ctx, 512)
+    vals, inv = np.unique(tri, return_inverse=True)                   # ascending similarities (inf last)
+    dist_rows = (len(vals) - inv).astype(np.float64)                  # highest similarity -> distance 1
+    # scipy wants the condensed matrix in (i < j) row-major order; ours is (i > j) by rows: reorder
+    ii, jj = np.tril_indices(k, -1)                                   # our order: pair (ii, jj), jj < ii
+    cond_index = k * jj - jj * (jj + 1) // 2 + (ii - jj - 1)          # position of (jj, ii) in scipy's order
+    cond = np.empty_like(dist_rows)
+    cond[cond_index] = dist_rows
+    Z = linkage(cond, method="single")
+    heights = vals[len(vals) - Z[:, 2].astype(np.int64)]              # back to similarities, descending
+    assert np.array_equal(heights, mw) and size[-1] == k
