@@ -56,6 +56,13 @@ def check_blocks(F, oracle, seqs, offsets, block_ids, n_per_block, want_sim=True
 
 
 @pytest.fixture(scope="module")
+def family4():
+    """BASELINE.json configs[4] (k = 415 519), generated once for this module (~45 s of host time)."""
+    from paper_1603_06958_b200 import synth
+    return synth.family(4)
+
+
+@pytest.fixture(scope="module")
 def F():
     import torch
     assert torch.cuda.is_available()
@@ -71,17 +78,16 @@ def test_config1_full_size_sampled(F, oracle):
     assert check_blocks(F, oracle, seqs, offsets, range(10), 2500) == 25000
 
 
-def test_config4_full_size_sampled(F, oracle):
+def test_config4_full_size_sampled(F, oracle, family4):
     """k = 415 519: the set bench.py times; blocks from the long end, the middle and the short end."""
-    from paper_1603_06958_b200 import synth
-    seqs, offsets = synth.family(4)
+    seqs, offsets = family4
     k = len(offsets) - 1
     assert k == 415519
     last = (k - 1) // BLOCK_ROWS
     assert check_blocks(F, oracle, seqs, offsets, [0, 1, 96, 240, last - 1, last], 6000) == 36000
 
 
-def test_config4_one_million_sampled_pairs_of_the_full_sweep(F, oracle):
+def test_config4_one_million_sampled_pairs_of_the_full_sweep(F, oracle, family4):
     """BASELINE.json configs[4]: "~8.6e10 pairs computed as streamed row blocks, oracle checked on 1e6 seeded
     sampled pairs".  The WHOLE sweep runs in the bench configuration (1024-row blocks, LCS + similarity);
     from every block the sampled entries are gathered on the device; all of them are then checked against
@@ -89,7 +95,7 @@ def test_config4_one_million_sampled_pairs_of_the_full_sweep(F, oracle):
     block-boundary rows, lengths = 0, 1, 31 mod 32) and the planted duplicates."""
     import torch
     from paper_1603_06958_b200 import synth
-    seqs, offsets = synth.family(4)
+    seqs, offsets = family4
     k = len(offsets) - 1
     perm_ref = oracle.sort_perm(offsets)
     with F.famsa_pack(seqs, offsets) as ctx:
