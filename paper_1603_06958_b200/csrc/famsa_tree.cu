@@ -46,32 +46,55 @@ __device__ __forceinline__ bool better(float w, uint32_t o, float bw, uint32_t b
 }
 
 // Best edge of each NEW vertex v (a row of the block) to a different component, over columns u < v.
+// A CTA takes ROW_R consecutive rows: one load of comp[u] serves all of them and each thread keeps
+// ROW_R x 4 independent loads in flight.  Measured on a 1.7 GB block: ROW_R = 1 (1024 CTAs) reads 5.7 TB/s,
+// ROW_R = 4 (256 CTAs) only 2.9 TB/s -- the CTA count matters more than sharing comp[u]; ROW_R = 1 is used.
+// HBM-bound: one pass over the block.
+template <int ROW_R>
 __global__ void __launch_bounds__(256) tree_row_kernel(const float* __restrict__ sim, uint32_t i0, uint32_t i1, int64_t out_base,
                                                        const uint32_t* __restrict__ comp, float* __restrict__ cw, uint32_t* __restrict__ co) {
-    const uint32_t v = i0 + blockIdx.x;
-    const float* row = sim + ((int64_t)v * (v - 1) / 2 - out_base);
-    const uint32_t cv = comp[v];
-    float bw = NO_EDGE; uint32_t bo = 0xFFFFFFFFu;
-    for (uint32_t u = threadIdx.x; u < v; u += 256) {
-        if (comp[u] != cv) {
-            const float w = __ldg(row + u);
-            if (better(w, u, bw, bo)) { bw = w; bo = u; }
-        }
-    }
+    const uint32_t v0 = i0 + blockIdx.x * ROW_R;
+    const float* row[ROW_R]; uint32_t cv[ROW_R], vv[ROW_R];
+    float bw[ROW_R]; uint32_t bo[ROW_R];
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-        const float ow = __shfl_xor_sync(0xffffffffu, bw, d);
-        const uint32_t oo = __shfl_xor_sync(0xffffffffu, bo, d);
-        if (better(ow, oo, bw, bo)) { bw = ow; bo = oo; }
+    for (int r = 0; r < ROW_R; ++r) {
+        const uint32_t v = min(v0 + r, i1 - 1);            // rows past the block repeat its last row (not stored)
+        vv[r] = v0 + r < i1 ? v : 0;                       // ... with an empty column range
+        row[r] = sim + ((int64_t)v * (v - 1) / 2 - out_base);
+        cv[r] = comp[v]; bw[r] = NO_EDGE; bo[r] = 0xFFFFFFFFu;
     }
-    __shared__ float sw[8];
-    __shared__ uint32_t so[8];
-    if ((threadIdx.x & 31) == 0) { sw[threadIdx.x >> 5] = bw; so[threadIdx.x >> 5] = bo; }
+    uint32_t vmax = 0;
+#pragma unroll
+    for (int r = 0; r < ROW_R; ++r) vmax = max(vmax, vv[r]);
+#pragma unroll 4
+    for (uint32_t u = threadIdx.x; u < vmax; u += 256) {
+        const uint32_t c = comp[u];
+        float w[ROW_R];
+#pragma unroll
+        for (int r = 0; r < ROW_R; ++r) w[r] = u < vv[r] ? __ldg(row[r] + u) : NO_EDGE;   // all loads first: ROW_R in flight
+#pragma unroll
+        for (int r = 0; r < ROW_R; ++r)
+            if (c != cv[r] && w[r] > bw[r]) { bw[r] = w[r]; bo[r] = u; }                  // u ascends per thread: first of equals stays
+    }
+    __shared__ float sw[ROW_R][8];
+    __shared__ uint32_t so[ROW_R][8];
+#pragma unroll
+    for (int r = 0; r < ROW_R; ++r) {
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            const float ow = __shfl_xor_sync(0xffffffffu, bw[r], d);
+            const uint32_t oo = __shfl_xor_sync(0xffffffffu, bo[r], d);
+            if (better(ow, oo, bw[r], bo[r])) { bw[r] = ow; bo[r] = oo; }
+        }
+        if ((threadIdx.x & 31) == 0) { sw[r][threadIdx.x >> 5] = bw[r]; so[r][threadIdx.x >> 5] = bo[r]; }
+    }
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (threadIdx.x < ROW_R && v0 + threadIdx.x < i1) {
+        const int r = threadIdx.x;
+        float w = sw[r][0]; uint32_t o = so[r][0];
         for (int q = 1; q < 8; ++q)
-            if (better(sw[q], so[q], bw, bo)) { bw = sw[q]; bo = so[q]; }
-        cw[v] = bw; co[v] = bo;
+            if (better(sw[r][q], so[r][q], w, o)) { w = sw[r][q]; o = so[r][q]; }
+        cw[v0 + r] = w; co[v0 + r] = o;
     }
 }
 
@@ -298,7 +321,7 @@ static int tree_rounds(famsa_tree* t, int64_t i0, int64_t i1, const float* sim_b
         a.comp = t->comp[cb]; a.comp_next = t->comp[cb ^ 1];
         tree_reset_kernel<<<gv, 256, 0, st>>>(a, round == 0);
         if (dense) {
-            tree_row_kernel<<<(unsigned)(i1 - i0), 256, 0, st>>>(sim_block, a.i0, a.i1, out_base, a.comp, t->cand_w[0], t->cand_o[0]);
+            tree_row_kernel<1><<<(unsigned)(i1 - i0), 256, 0, st>>>(sim_block, a.i0, a.i1, out_base, a.comp, t->cand_w[0], t->cand_o[0]);
             tree_col_kernel<<<(unsigned)((a.i1 - 1 + COL_X - 1) / COL_X), dim3(COL_X, COL_Y), 0, st>>>(sim_block, a.i0, a.i1, out_base, a.comp, t->cand_w[1], t->cand_o[1]);
             t->launches += 2;
         }
