@@ -31,7 +31,9 @@ sys.path.insert(0, ROOT)
 METRIC = "all_pairs_lcs_gcups"
 UNIT = "GCUPS"
 BLOCK_ROWS = 1024
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 3.387e9   # profiles/r01_ncu_sweep_short_v2_config4.md (ncu --set full, one <10> launch)
+# DRAM traffic of ONE configs[4] step (all its sweep launches), dram__bytes_read.sum + dram__bytes_write.sum per launch
+# from ncu, summed: profiles/r02_ncu_step_traffic.md.  Not measurable outside a profiler, so a recorded figure.
+NCU_STEP_TRAFFIC = {"config": 4, "bytes": None, "launches": None, "source": "profiles/r02_ncu_step_traffic.md"}
 ALU_INSTR_PER_CELL = 3.0 / 32.0      # LOP3 + IADD3.X + LOP3 per 32-bit word-step
 WORKLOADS = {
     0: "configs[0]: k=500, one family, all 124750 pairs",
@@ -58,6 +60,8 @@ def parse_args():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--guide-tree", action="store_true",
                     help="also time stages I+II (full sweep + single-linkage guide tree), the whole job dealt over the ranks")
+    ap.add_argument("--no-guide-tree", action="store_true", help="skip the stages I+II leg that N=1 runs by default")
+    ap.add_argument("--tune", default=None, help="rows_per_cta,small_job_mode,l2_group_mb for famsa_ctx_set_tuning (experiments)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU work per oracle sample")
     return ap.parse_args()
 
@@ -117,7 +121,7 @@ class ClockSampler:
 def oracle_sample(seqs, offsets, blocks, cpu_seconds, seed, n=400000):
     """A bounded seeded sample of the step's pairs for the CPU oracle: uniform over the pairs of
     the step's row blocks, cut where the cell count reaches ~cpu_seconds of work on all cores
-    (planning rate 0.3 GCUPS per core).  Returns (orig_i, orig_j, cells, cores)."""
+    (planning rate 0.3 GCUPS per core).  Returns (orig_i, orig_j, cells, cores, sorted_i, sorted_j)."""
     from oracle import famsa_oracle
     cores = famsa_oracle.n_threads_default()
     perm = famsa_oracle.sort_perm(offsets)
@@ -125,7 +129,7 @@ def oracle_sample(seqs, offsets, blocks, cpu_seconds, seed, n=400000):
     rows = np.concatenate([np.arange(max(a, 1), b, dtype=np.int64) for a, b in blocks]) if blocks else np.zeros(0, np.int64)
     if rows.size == 0:
         z = np.zeros(0, np.int64)
-        return z, z, 0.0, cores
+        return z, z, 0.0, cores, z, z
     rng = np.random.default_rng(seed)
     i = rng.choice(rows, size=n, p=rows / rows.sum())
     j = (rng.random(n) * i).astype(np.int64)
@@ -133,7 +137,53 @@ def oracle_sample(seqs, offsets, blocks, cpu_seconds, seed, n=400000):
     budget = 0.3e9 * cores * cpu_seconds
     cut = int(np.searchsorted(np.cumsum(cells), budget)) + 1
     cut = min(cut, n)
-    return perm[i[:cut]], perm[j[:cut]], float(cells[:cut].sum()), cores
+    return perm[i[:cut]], perm[j[:cut]], float(cells[:cut].sum()), cores, i[:cut], j[:cut]
+
+
+def time_bitparallel(seqs, offsets, blocks, seconds, seed):
+    """CONTEXT figure: the paper's own CPU design (64-bit bit-parallel LCS, several pairs per SIMD register,
+    rows over threads; oracle/bitpar_cpu.c) on a bounded sample of the step: seeded rows of the step's row
+    blocks, 64 seeded columns j < i each (the row's match table is built once, as in the paper's design).
+    Every ISA variant the host runs is timed after a pilot that sizes the sample for ~`seconds` of work."""
+    from oracle import famsa_oracle
+    cores = famsa_oracle.n_threads_default()
+    perm = famsa_oracle.sort_perm(offsets)
+    lens = np.diff(offsets)[perm].astype(np.int64)
+    rows_all = np.concatenate([np.arange(max(a, 64), b, dtype=np.int64) for a, b in blocks if b > 64]) if blocks else np.zeros(0, np.int64)
+    if rows_all.size == 0:
+        return None
+    rng = np.random.default_rng(seed)
+    ncol = 64
+
+    def sample(n_rows):
+        ri = rng.choice(rows_all, size=n_rows, p=rows_all / rows_all.sum())
+        cj = (rng.random((n_rows, ncol)) * ri[:, None]).astype(np.int64)
+        cells = float((lens[ri][:, None] * lens[cj]).sum())
+        col_ptr = np.arange(n_rows + 1, dtype=np.int64) * ncol
+        return perm[ri], col_ptr, perm[cj].ravel(), cells
+
+    best = famsa_oracle.bitpar_best_isa()
+    variants = [0, 2] + ([14] if best in (14, 18) else []) + ([18] if best == 18 else [])
+    out = {}
+    for isa in variants:
+        ri, cp, cj, cells = sample(256 * cores)                       # pilot
+        t0 = time.perf_counter()
+        famsa_oracle.bitpar_rowsets(seqs, offsets, ri, cp, cj, isa=isa)
+        rate = cells / max(time.perf_counter() - t0, 1e-6)
+        n_rows = int(min(max(rate * seconds / (cells / (256 * cores)), 256 * cores), 4_000_000 // ncol))
+        ri, cp, cj, cells = sample(n_rows)
+        t0 = time.perf_counter()
+        famsa_oracle.bitpar_rowsets(seqs, offsets, ri, cp, cj, isa=isa)
+        dt = time.perf_counter() - t0
+        out[isa] = {"gcups": cells / dt / 1e9, "pairs_per_s": n_rows * ncol / dt, "seconds": dt, "pairs": n_rows * ncol, "cells": cells}
+    top = max(out, key=lambda q: out[q]["gcups"])
+    return {"value": out[top]["gcups"], "unit": UNIT, "cores": cores, "isa": famsa_oracle.BITPAR_ISA_NAMES[top],
+            "kind": "context: the paper's own CPU design (PAPER.md:44, 54-56: 64-bit bit-parallel LCS, `a` pairs per SIMD "
+                    "register, rows over threads; oracle/bitpar_cpu.c) -- not a parity oracle",
+            "pairs_per_s": out[top]["pairs_per_s"],
+            "sample": "%d seeded rows of the step's row blocks x %d seeded columns (%.3g cells, %.1f s)" % (
+                out[top]["pairs"] // ncol, ncol, out[top]["cells"], out[top]["seconds"]),
+            "variants_gcups": {famsa_oracle.BITPAR_ISA_NAMES[q]: round(v["gcups"], 2) for q, v in out.items()}}
 
 
 def time_oracle(seqs, offsets, pi, pj, want_sim):
@@ -156,7 +206,7 @@ def run_reference(args, rank, world):
     secs = min(args.cpu_seconds, 8.0)
     times, cells_step, pairs_step, cores = [], 0.0, 0, 1
     for s in range(args.warmup + args.steps):
-        pi, pj, cells, cores = oracle_sample(seqs, offsets, blocks, secs, seed=1000 + s)
+        pi, pj, cells, cores, _, _ = oracle_sample(seqs, offsets, blocks, secs, seed=1000 + s)
         dt = time_oracle(seqs, offsets, pi, pj, want_sim)
         if s >= args.warmup:
             times.append(dt); cells_step += cells; pairs_step += pi.size
@@ -172,7 +222,11 @@ def run_reference(args, rank, world):
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
+        "note": "the reference arm is the plain-DP oracle, as the task contract states; the paper's own method on "
+                "these cores (bit-parallel, multi-pair SIMD) is `cpu_bitparallel` -- divide by that for an honest speed-up",
     }
+    if not args.no_cpu:
+        line["cpu_bitparallel"] = time_bitparallel(seqs, offsets, blocks, min(args.cpu_seconds, 6.0), seed=11)
     print(json.dumps(line), flush=True)
 
 
@@ -225,6 +279,32 @@ def gather_forests(dist, a, b, w, k, device):
     return out
 
 
+def gather_sampled(F, torch, ctx, blocks, si, sj, bufs, ck, stream):
+    """One un-timed pass over the step's row blocks that (a) accumulates each block's checksum into ck[n]
+    and (b) picks the sampled entries (sorted pair indices si > sj, any order) out of each block while it
+    sits in its ping-pong buffer.  Returns (lcs int64, sim float64) numpy arrays parallel to si."""
+    dev = bufs[0][0].device
+    order = np.argsort(si, kind="stable")
+    si_s, sj_s = si[order], sj[order]
+    got_l = torch.zeros(si.size, dtype=torch.int16, device=dev)
+    got_s = torch.zeros(si.size, dtype=torch.float32, device=dev)
+    pos_all = torch.from_numpy(si_s * (si_s - 1) // 2 + sj_s).to(dev)
+    for n, (a, b) in enumerate(blocks):
+        lcs, sim = bufs[n & 1]
+        F.famsa_lcs_rows_checksum(ctx, a, b, lcs, sim, ck[n], stream)
+        lo, hi = int(np.searchsorted(si_s, a)), int(np.searchsorted(si_s, b))
+        if hi > lo:
+            idx = pos_all[lo:hi] - a * (a - 1) // 2
+            got_l[lo:hi] = lcs.view(torch.int16)[idx]
+            if sim is not None:
+                got_s[lo:hi] = sim[idx]
+    torch.cuda.synchronize()
+    gl = np.empty(si.size, np.int64); gs = np.empty(si.size, np.float64)
+    gl[order] = got_l.cpu().numpy().view(np.uint16).astype(np.int64)
+    gs[order] = got_s.cpu().numpy().astype(np.float64)
+    return gl, gs
+
+
 def run_cuda(args, rank, world, local_rank):
     import torch
     from paper_1603_06958_b200 import famsa as F, synth
@@ -245,11 +325,14 @@ def run_cuda(args, rank, world, local_rank):
         blocks = step_blocks(k, stride)[:1]       # more ranks than blocks: repeat one block rather than idle (reported cells stay true)
 
     peak0 = F.famsa_alu_peak(local_rank)
+    mix0 = F.famsa_mix_peak(local_rank)
     t0 = time.perf_counter()
     ctx = F.famsa_pack(seqs, offsets, device=local_rank)
     torch.cuda.synchronize()
     pack_ms = (time.perf_counter() - t0) * 1e3
     pack_launches = F.famsa_launch_count(ctx)
+    if args.tune:
+        F.famsa_ctx_set_tuning(ctx, *[int(x) for x in args.tune.split(",")])
 
     max_pairs = max(F.famsa_rows_pairs(a, b) for a, b in blocks)
     bufs = [(torch.empty(max_pairs, dtype=torch.uint16, device=dev),
@@ -257,11 +340,14 @@ def run_cuda(args, rank, world, local_rank):
     cells_step = sum(F.famsa_rows_cells(ctx, a, b) for a, b in blocks)
     pairs_step = sum(F.famsa_rows_pairs(a, b) for a, b in blocks)
     stream = torch.cuda.current_stream()
+    # one 64-bit checksum pair per row block, accumulated by the sweep's own epilogue in every timed step
+    # ("a 64-bit checksum per block is kept to prove the work was done")
+    ck = torch.zeros((len(blocks), 2), dtype=torch.int64, device=dev)
 
     def step():
         for n, (a, b) in enumerate(blocks):
             lcs, sim = bufs[n & 1]                            # ping-pong: the consumer owns one block while the next is swept
-            F.famsa_lcs_rows(ctx, a, b, lcs, sim, stream)
+            F.famsa_lcs_rows_checksum(ctx, a, b, lcs, sim, ck[n], stream)
 
     def barrier():
         if dist is not None:
@@ -270,6 +356,8 @@ def run_cuda(args, rank, world, local_rank):
 
     for _ in range(args.warmup):
         step()
+    barrier()
+    ck.zero_()
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
@@ -284,9 +372,35 @@ def run_cuda(args, rank, world, local_rank):
     launches = F.famsa_launch_count(ctx) - l0
     ms_total = ev[0].elapsed_time(ev[-1])
     step_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)]
+    ms_rank = ms_total
     ms_total, cells_all, pairs_all = reduce_over_ranks(dist, ms_total, cells_step, pairs_step, dev)
     sec = ms_total * 1e-3
     value = cells_all * args.steps / sec / 1e9
+    ck_timed = ck.cpu().numpy().astype(np.uint64)
+
+    # ---- was the timed work right?  One more (un-timed) pass: fresh checksums + the entries of the oracle's
+    # sample gathered from the row blocks; the comparison with the oracle happens in the cpu_baseline leg
+    sample = None
+    if rank == 0 and not args.no_cpu:
+        sample = oracle_sample(seqs, offsets, blocks, args.cpu_seconds, seed=7)
+    ck1 = torch.zeros_like(ck)
+    si = sample[4] if sample is not None else np.zeros(0, np.int64)
+    sj = sample[5] if sample is not None else np.zeros(0, np.int64)
+    gpu_l, gpu_s = gather_sampled(F, torch, ctx, blocks, si, sj, bufs, ck1, stream)
+    ck_once = ck1.cpu().numpy().astype(np.uint64)
+    checksum = {"blocks": len(blocks), "lcs_sum_step": int(ck_once[:, 0].sum()), "sim_bits_sum_step": int(ck_once[:, 1].sum() & np.uint64(2**64 - 1)),
+                "timed_steps_equal_steps_x_one_pass": bool(np.array_equal(ck_timed, ck_once * np.uint64(args.steps)))}
+    # the last two blocks still sit in the ping-pong buffers: reduce them with torch (independent of the kernels)
+    indep = True
+    for n in range(max(0, len(blocks) - 2), len(blocks)):
+        a, b = blocks[n]
+        npairs = F.famsa_rows_pairs(a, b)
+        lcs, sim = bufs[n & 1]
+        sl = int((lcs.view(torch.int16)[:npairs].to(torch.int64) & 0xFFFF).sum().item())
+        indep &= sl == int(ck_once[n, 0])
+        if sim is not None:
+            indep &= int(sim[:npairs].view(torch.int32).to(torch.int64).sum().item()) == int(ck_once[n, 1])
+    checksum["last_blocks_equal_torch_reduction"] = bool(indep)
 
     # ---- e2e: HOST buffers through the C ABI; pack (H2D of the residues) + sweep + D2H every step
     # (one call over all rows when the whole result fits 2 GB of pinned memory, else one call per row block
@@ -299,14 +413,25 @@ def run_cuda(args, rank, world, local_rank):
     h_sim2 = [h_sim, h_sim if (one_call or not want_sim) else torch.empty(e2e_pairs, dtype=torch.float32).pin_memory()]
     # long steps: 2 timed e2e steps; short steps (small configs) are noisy (allocations in pack): more of them
     e2e_steps = max(1, min(args.steps, 2)) if ms_total / args.steps > 500.0 else max(2, min(2 * args.steps, 10))
-    def e2e_step():
+    phases = {"pack_ms": 0.0, "sweep_ms": 0.0, "d2h_ms": 0.0, "d2h_bytes": 0.0, "span_ms": 0.0, "chunks": 0}
+
+    def e2e_step(profile=False):
+        t_p = time.perf_counter()
         c2 = F.famsa_pack(seqs, offsets, device=local_rank)
+        if args.tune:
+            F.famsa_ctx_set_tuning(c2, *[int(x) for x in args.tune.split(",")])
+        phases["pack_ms"] += (time.perf_counter() - t_p) * 1e3 if profile else 0.0
+        if profile:
+            F.famsa_host_profile(c2, True)
         if one_call:
             F.famsa_lcs_rows_host(c2, 0, k, h_lcs, h_sim)
         else:
             for n, (a, b) in enumerate(blocks):               # two pinned row-block buffers, copies overlap the next sweep
                 F.famsa_lcs_rows_host_async(c2, a, b, h_lcs2[n & 1], h_sim2[n & 1] if want_sim else None)
             F.famsa_sync(c2)
+        if profile:
+            for key, v in F.famsa_host_profile_read(c2).items():
+                phases[key] += v
         c2.free()
     e2e_step()                                                # warm-up (allocations, staging buffers)
     if ms_total / args.steps <= 500.0:
@@ -324,6 +449,14 @@ def run_cuda(args, rank, world, local_rank):
     e2e_value = cells_all * e2e_steps / e2e_sec / 1e9
     h2d = int(seqs.nbytes + offsets.nbytes)
     d2h = int(pairs_step * (2 + (4 if want_sim else 0)))
+    # one more e2e step, un-timed, with the per-phase CUDA events switched on (they serialise nothing, but
+    # the step is kept out of the timed region anyway)
+    t_w = time.perf_counter()
+    e2e_step(profile=True)
+    phases["wall_ms"] = (time.perf_counter() - t_w) * 1e3
+    if phases["d2h_ms"] > 0:
+        phases["d2h_gb_per_s"] = phases["d2h_bytes"] / phases["d2h_ms"] / 1e6
+    F.famsa_trim()                                            # hand the pooled staging back before the big buffers below
 
     # ---- one full sweep, timed alone (N = 1, configs 3-4 only: the other configs' step already is one)
     full = None
@@ -346,7 +479,7 @@ def run_cuda(args, rank, world, local_rank):
         full = {"ms": fms, "gcups": fcells / fms / 1e6, "pairs": F.famsa_rows_pairs(0, k),
                 "pairs_per_s": F.famsa_rows_pairs(0, k) / fms * 1e3, "cells": fcells}
     tree = None
-    if args.guide_tree:
+    if args.guide_tree or (world == 1 and want_sim and not args.no_guide_tree):
         # stages I + II, the WHOLE job dealt over the ranks (strong scaling): rank r sweeps row blocks
         # r, r + N, ... and keeps their spanning forest; one all_gather of the forests' edges; rank 0 merges
         bufs = None
@@ -355,14 +488,17 @@ def run_cuda(args, rank, world, local_rank):
         l1 = F.famsa_launch_count(ctx)
         t0 = time.perf_counter()
         forest = F.famsa_guide_forest(ctx, BLOCK_ROWS, rank, world)
+        t_forest = time.perf_counter() - t0
         fa, fb, fw = F.famsa_tree_edges(forest)
         parts = gather_forests(dist, fa, fb, fw, k, dev)
         n_merges = 0
+        t1 = time.perf_counter()
         if rank == 0:
             for r in range(1, world):
                 F.famsa_tree_merge_edges(forest, *parts[r])
             ia, ib, mw, msize = F.famsa_tree_finish(forest)
             n_merges = int(mw.size)
+        t_finish = time.perf_counter() - t1
         barrier()
         dt = time.perf_counter() - t0
         forest.free()
@@ -373,57 +509,75 @@ def run_cuda(args, rank, world, local_rank):
         fcells = F.famsa_rows_cells(ctx, 0, k)
         if rank == 0:
             tree = {"seconds": dt, "gcups_equivalent": fcells / dt / 1e9, "launches_rank0": F.famsa_launch_count(ctx) - l1,
+                    "forest_seconds_rank0": t_forest, "merge_and_dendrogram_seconds": t_finish,
                     "merges": n_merges, "top_similarity": float(mw[0]) if mw.size else None,
                     "last_similarity": float(mw[-1]) if mw.size else None, "scaling": "strong", "n_gpus": world,
                     "what": "famsa_guide_forest per rank (cyclic deal of all 1024-row blocks: sweep, fp32 similarity only, + incremental "
                             "single-linkage forest), all_gather of the forests' edges, merge + dendrogram on rank 0; wall clock, max over ranks"}
     peak1 = F.famsa_alu_peak(local_rank)
+    mix1 = F.famsa_mix_peak(local_rank)
     ctx.free()
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
 
-    # ---- rank 0: the oracle beside it, the roofline, the line
+    # ---- rank 0: the oracle beside it (and against it), the roofline, the line
     cpu = None
-    if not args.no_cpu:
-        pi, pj, ccells, cores = oracle_sample(seqs, offsets, blocks, args.cpu_seconds, seed=7)
-        dt = time_oracle(seqs, offsets, pi, pj, want_sim)
+    parity = None
+    if sample is not None:
+        pi, pj, ccells, cores = sample[:4]
+        from oracle import famsa_oracle
+        t0 = time.perf_counter()
+        lref, sref = famsa_oracle.pairs(seqs, offsets, pi, pj, want_sim=want_sim)
+        dt = time.perf_counter() - t0
         cpu = {"value": ccells / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
                "pairs_per_s": pi.size / dt,
                "sample": "%d seeded uniform pairs of the step's row blocks (%.3g cells, %.1f s)" % (pi.size, ccells, dt)}
+        # the same pairs, as the GPU stored them in the step's row blocks
+        mism = int((gpu_l != lref).sum())
+        rel = 0.0
+        inf_ok = True
+        if want_sim:
+            fin = np.isfinite(sref)
+            inf_ok = bool(np.array_equal(np.isinf(gpu_s), ~fin))
+            if fin.any():
+                rel = float(np.max(np.abs(gpu_s[fin] - sref[fin]) / np.abs(sref[fin])))
+        parity = {"pairs": int(pi.size), "lcs_mismatch": mism, "sim_max_rel_err": rel, "inf_match": inf_ok,
+                  "what": "the cpu_baseline sample's oracle results vs the entries the CUDA path stored for the same pairs"}
     cpu_bp = None
     if not args.no_cpu:
-        from oracle import famsa_oracle
-        pi, pj, ccells, cores = oracle_sample(seqs, offsets, blocks, args.cpu_seconds * 6, seed=11, n=6000000)   # ~50x faster than the DP
-        t0 = time.perf_counter()
-        famsa_oracle.bitpar_pairs(seqs, offsets, pi, pj)
-        dt = time.perf_counter() - t0
-        cpu_bp = {"value": ccells / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "context: the paper's own CPU design "
-                  "(64-bit bit-parallel LCS, one pair per task over threads, scalar; oracle/bitpar_cpu.c) -- not a parity oracle",
-                  "pairs_per_s": pi.size / dt, "sample": "%d seeded uniform pairs (%.3g cells, %.1f s)" % (pi.size, ccells, dt)}
+        cpu_bp = time_bitparallel(seqs, offsets, blocks, min(args.cpu_seconds, 6.0), seed=11)
     p_int = max(peak0["instr_per_s"], peak1["instr_per_s"])          # measured INT32 ALU-pipe rate (thread-instr/s)
     sm_count = torch.cuda.get_device_properties(local_rank).multi_processor_count
-    achieved = cells_step * args.steps * ALU_INSTR_PER_CELL / (ev[0].elapsed_time(ev[-1]) * 1e-3)   # this rank's stream
+    achieved = cells_step * args.steps * ALU_INSTR_PER_CELL / (ms_rank * 1e-3)   # this rank's stream
     peaks_file = os.path.join(ROOT, "MEASURED_PEAKS.json")
     sm_max = 1965.0
     if os.path.exists(peaks_file):
         sm_max = float(json.load(open(peaks_file)).get("sm_max_mhz", sm_max))
     nominal = sm_count * 64 * sm_max * 1e6
+    out_bytes = pairs_step * (2 + (4 if want_sim else 0))
+    traffic = None
+    traffic_note = "dram__bytes_* need a profiler; no recorded capture for this config (see profiles/)"
+    if NCU_STEP_TRAFFIC["bytes"] and args.config == NCU_STEP_TRAFFIC["config"] and stride == 16 and world == 1:
+        traffic = NCU_STEP_TRAFFIC["bytes"] / NCU_STEP_TRAFFIC["launches"]
+        traffic_note = ("dram__bytes_read.sum + dram__bytes_write.sum summed over the %d sweep launches of one step of this workload "
+                        "(%.3g B) / launches, recorded in %s; the step's algorithmic output is %.3g B" % (
+                            NCU_STEP_TRAFFIC["launches"], NCU_STEP_TRAFFIC["bytes"], NCU_STEP_TRAFFIC["source"], out_bytes))
     roofline = {
         "bound": "alu", "achieved": achieved / 1e12, "peak": p_int / 1e12, "unit": "TIOP/s (int32 ALU-pipe lane-instr)",
-        "frac": achieved / p_int, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
-        "traffic_note": "dram__bytes_read+write of ONE sweep_short_kernel<10> launch (1.68e8 pairs of configs[4]), "
-                        "from profiles/r01_ncu_sweep_short_v2_config4.md; not measured in this run",
-        "kernel": "famsa::sweep_short_kernel<W> (%d launches per step)" % (launches // max(args.steps, 1)),
+        "frac": achieved / p_int, "traffic": traffic, "traffic_note": traffic_note,
+        "traffic_step_over_algorithmic": (NCU_STEP_TRAFFIC["bytes"] / out_bytes) if traffic else None,
+        "kernel": "famsa::sweep_short_kernel<W,NR> (%d launches per step)" % (launches // max(args.steps, 1)),
         "algorithmic_instr_per_cell": ALU_INSTR_PER_CELL,
         "peak_source": "famsa_alu_peak micro-kernel, measured in this run (MEASURED_PEAKS.json has no integer peak)",
         "peak_instr_per_clk_sm": max(peak0["instr_per_clk_sm"], peak1["instr_per_clk_sm"]),
         "peak_sm_mhz": max(peak0["sm_mhz"], peak1["sm_mhz"]),
+        "mix_ceiling_instr_per_clk_sm": max(mix0["alu_instr_per_clk_sm"], mix1["alu_instr_per_clk_sm"]),
+        "mix_note": "famsa_mix_peak: the same micro-kernel with the sweep's mix (3 ALU + 1 conflict-free LDS.32 per word-step)",
         "frac_of_nominal_64_per_clk_sm_at_max_clock": achieved / nominal,
         "roofline_gcups": p_int / ALU_INSTR_PER_CELL / 1e9,
     }
-    out_bytes = pairs_step * (2 + (4 if want_sim else 0))
     if out_bytes > 126e6:
         l2_note = "no flush needed: every step writes %.2f GB of row-block output (> 126 MB L2) between re-reads" % (out_bytes / 1e9)
     else:
@@ -441,9 +595,13 @@ def run_cuda(args, rank, world, local_rank):
         "step_ms": step_ms, "pack_ms": pack_ms,
         "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"], "samples": clocks["samples"]},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
-                "what": "famsa_pack from host memory + famsa_lcs_rows_host into a pinned host row-block buffer, every step"},
+                "frac_of_device_resident": e2e_value / value,
+                "what": "famsa_pack from host memory + famsa_lcs_rows_host into a pinned host row-block buffer, every step",
+                "phases_of_one_untimed_step": phases},
         "gpu_launches": launches,
         "roofline": roofline,
+        "checksum": checksum,
+        "parity_in_bench": parity,
         "cpu_baseline": cpu,
         "cpu_bitparallel": cpu_bp,
         "output_gb_per_s": pairs_all * args.steps * (2 + (4 if want_sim else 0)) / sec / 1e9,
@@ -455,6 +613,12 @@ def run_cuda(args, rank, world, local_rank):
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+    ok = checksum["timed_steps_equal_steps_x_one_pass"] and checksum["last_blocks_equal_torch_reduction"]
+    if parity is not None:
+        ok = ok and parity["lcs_mismatch"] == 0 and parity["inf_match"] and parity["sim_max_rel_err"] <= 1e-6
+    if not ok:
+        sys.stderr.write("bench.py: the timed work FAILED its self-check (checksum / parity_in_bench above)\n")
+        sys.exit(3)
 
 
 def main():

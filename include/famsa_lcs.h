@@ -101,6 +101,40 @@ int famsa_lcs_rows_host_async(famsa_ctx* ctx, int64_t i0, int64_t i1,
 /* Wait for everything the host path of this ctx has enqueued. */
 int famsa_sync(famsa_ctx* ctx);
 
+/*
+ * famsa_lcs_rows_checksum -- famsa_lcs_rows plus a 64-bit checksum of what the call stored (SURVEY.md 8(d):
+ * "a 64-bit checksum per block is kept to prove the work was done"), accumulated by the sweep kernels' own
+ * epilogue (warp reductions + one atomic per warp and row; nothing is re-read):
+ *   checksum_dev  DEVICE  uint64[2], ADDED to (the caller zeroes it):
+ *                         [0] += sum of the LCS lengths of the call's pairs,
+ *                         [1] += sum of the fp32 similarities' bit patterns (untouched if sim_out is NULL).
+ * Both are order-independent integer sums mod 2^64, so any reduction over the output arrays reproduces them.
+ */
+int famsa_lcs_rows_checksum(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_out, float* sim_out,
+                            uint64_t* checksum_dev, void* cuda_stream);
+
+/*
+ * Per-phase timing of the HOST-output path (diagnostics for the end-to-end number).
+ *   famsa_host_profile(ctx, 1)   from now on every row chunk of famsa_lcs_rows_host* is bracketed by CUDA
+ *                                events on the ctx's compute and copy streams.
+ *   famsa_host_profile_read      waits for the ctx's host path, then fills HOST out[5] and resets:
+ *                                [0] sum of the chunks' sweep times (ms), [1] sum of their device->host copy
+ *                                times (ms), [2] bytes copied, [3] first sweep start -> last copy end (ms),
+ *                                [4] number of chunks.
+ *   famsa_pack_profile           HOST ms4[4]: wall time of famsa_pack's phases for this ctx: host->device copy +
+ *                                encode, length sort, host-side plan, device allocation + stream/table build.
+ */
+int famsa_host_profile(famsa_ctx* ctx, int enable);
+int famsa_host_profile_read(famsa_ctx* ctx, double* out5);
+int famsa_pack_profile(const famsa_ctx* ctx, double* ms4);
+
+/*
+ * The HOST-output path keeps its device staging (two row-chunk buffers, two streams) in a process-wide pool:
+ * famsa_free returns a ctx's set to the pool and the next ctx on that device reuses it.  famsa_trim()
+ * releases every idle set (call it before a large allocation of your own).
+ */
+int famsa_trim(void);
+
 /* Number of (i, j < i) entries of rows [i0, i1): i1(i1-1)/2 - i0(i0-1)/2.  -1 if i0 > i1 or i0 < 0. */
 int64_t famsa_rows_pairs(int64_t i0, int64_t i1);
 
@@ -132,6 +166,16 @@ int64_t famsa_launch_count(const famsa_ctx* ctx);
  *   sm_mhz            HOST out: SM clock achieved during the run (clock64 / elapsed time)
  */
 int famsa_alu_peak(int device, double* instr_per_s, double* instr_per_clk_sm, double* sm_mhz);
+
+/*
+ * famsa_mix_peak -- the same micro-benchmark with the sweep's instruction mix: per word-step 3 ALU-pipe
+ * instructions (LOP3, IADD3.X, LOP3) plus ONE conflict-free 32-bit shared-memory load, V in registers,
+ * no global traffic, 40 warps per SM.  What it reaches is the ceiling of this mix on the SM's issue
+ * logic; bench.py prints it beside the ALU peak (roofline.mix_ceiling_instr_per_clk_sm).
+ *   alu_instr_per_clk_sm  HOST out: ALU-pipe thread-instructions per clock per SM achieved (the 3 per word-step)
+ *   sm_mhz                HOST out: SM clock during the run
+ */
+int famsa_mix_peak(int device, double* alu_instr_per_clk_sm, double* sm_mhz);
 
 
 /* ---------------------------------------------------------------------------------------------
@@ -200,8 +244,16 @@ int famsa_guide_tree(famsa_ctx* ctx, int64_t block_rows, int64_t* id_a_host, int
  */
 int famsa_guide_forest(famsa_ctx* ctx, int64_t block_rows, int64_t part, int64_t parts, famsa_tree** out);
 
-/* Tuning knob (process-wide, tests sweep it): rows of A per CTA on the register path, 1..12. */
-int famsa_set_tuning(int rows_per_cta);
+/*
+ * Tuning knobs of ONE ctx (tests sweep them; concurrent calls on other ctxs are unaffected).  Results never
+ * depend on them.  0 (or -1 for small_job_mode) restores the default.
+ *   rows_per_cta    rows of A per CTA on the register path, 1..12 (default 2)
+ *   small_job_mode  -1 auto: calls with fewer than 2048 x SM-count pairs run one pair per thread in one-warp
+ *                   CTAs (the hardware then balances the job at warp granularity); 0 never; 1 always
+ *   l2_group_mb     size of the residue-stream slice that one column group of a launch re-reads from L2
+ *                   (default 24)
+ */
+int famsa_ctx_set_tuning(famsa_ctx* ctx, int rows_per_cta, int small_job_mode, int l2_group_mb);
 
 void famsa_free(famsa_ctx* ctx);            /* famsa_free(NULL) is a no-op */
 const char* famsa_strerror(int code);       /* static text for a FAMSA_E* code */

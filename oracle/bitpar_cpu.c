@@ -1,12 +1,16 @@
 /*
  * bitpar_cpu.c -- CONTEXT BASELINE for bench.py, NOT a parity oracle and NOT product code.
  *
- * The paper's own stage-I design on a CPU (PAPER.md:44, 54): the bit-parallel LCS length with
- * w = 64-bit words, one pair per task, spread over threads (the paper additionally packs several
- * pairs into AVX registers; this scalar version does not).  It exists so that the benchmark can put
- * "the paper's method on this box's host cores" beside the GPU number, because the paper prints no
- * stage-I throughput.  It shares the recurrence with the CUDA path, so it proves nothing about
- * parity; it is itself checked against the plain-DP oracle in tests/test_oracle_pins.py.
+ * The paper's own stage-I design on a CPU (PAPER.md:44, 54-56): the bit-parallel LCS length with
+ * w = 64-bit words, the pairs spread over threads, and "multiple pairs of sequences ... processed
+ * simultaneously by the same thread" in SIMD registers -- a = 2 (128-bit), 4 (AVX2) or 8 (AVX-512)
+ * 64-bit words per vector.  One task = one ROW sequence A (its match bit-vectors are built once) against
+ * a list of column sequences B, `a` of them at a time: lane l of every vector belongs to pair (A, B_l);
+ * the add carry between words is a per-lane mask obtained by unsigned compares.
+ * It exists so that the benchmark can put "the paper's method on this box's host cores" beside the GPU
+ * number, because the paper prints no stage-I throughput.  It shares the recurrence with the CUDA path,
+ * so it proves nothing about parity; it is itself checked against the plain-DP oracle in
+ * tests/test_oracle_pins.py (every lane count, through the generic code path where the host lacks the ISA).
  * Shares no code with paper_1603_06958_b200/csrc.  Build: gcc -O2 (oracle/build.py).
  */
 #include <stdint.h>
@@ -15,72 +19,166 @@
 #include <pthread.h>
 
 #define SYMS 32
+#define PAD_SYM 31           /* never a residue code (codes are < 25): its match words are all zero */
 
-/* LCS length of a (length la, the side that carries the bit-vector) and b; codes < 32. */
-static int32_t bitpar_lcs(const uint8_t *a, int32_t la, const uint8_t *b, int32_t lb, uint64_t *M, uint64_t *V)
+/* Match bit-vectors of a, layout M[word][symbol] (one row of 32 words per 64 residues). */
+static void build_table(const uint8_t *a, int32_t la, int32_t W, uint64_t *M)
 {
-    int32_t W = (la + 63) / 64, i, j, w, lcs = 0;
+    int32_t i;
     memset(M, 0, sizeof(uint64_t) * SYMS * (size_t)W);
-    for (i = 0; i < la; ++i) M[(size_t)a[i] * W + (i >> 6)] |= 1ull << (i & 63);
+    for (i = 0; i < la; ++i) M[(size_t)(i >> 6) * SYMS + a[i]] |= 1ull << (i & 63);
+}
+
+/* scalar: one pair.  LCS length of the table's sequence (W words) and b. */
+static int32_t lcs_scalar(const uint64_t *M, int32_t W, const uint8_t *b, int32_t lb, uint64_t *V)
+{
+    int32_t j, w, lcs = 0;
     for (w = 0; w < W; ++w) V[w] = ~0ull;
     for (j = 0; j < lb; ++j) {
-        const uint64_t *m = M + (size_t)b[j] * W;
+        const uint64_t *m = M + b[j];
         unsigned long long carry = 0;
         for (w = 0; w < W; ++w) {
-            uint64_t u = V[w] & m[w];
+            uint64_t mw = m[(size_t)w * SYMS];
+            uint64_t u = V[w] & mw;
             uint64_t t = V[w] + u;                      /* add with carry in and out, across words */
             uint64_t s = t + carry;
             carry = (unsigned long long)((t < u) | (s < t));
-            V[w] = s | (V[w] & ~m[w]);
+            V[w] = s | (V[w] & ~mw);
         }
     }
     for (w = 0; w < W; ++w) lcs += __builtin_popcountll(~V[w]);
     return lcs;
 }
 
+/* SIMD: N pairs (one table, N column sequences) per vector of N 64-bit lanes.  V: N*W words of scratch
+ * (vector-aligned).  Columns shorter than the group's longest are padded with PAD_SYM (a no-op step).
+ * The body is written once with GCC vector extensions and instantiated per lane count and target ISA. */
+#define DEFINE_LCS_VEC(NAME, N, TARGET)                                                                   \
+    typedef uint64_t NAME##_vec __attribute__((vector_size(8 * N)));                                      \
+    TARGET static void NAME(const uint64_t *M, int32_t W, const uint8_t *const *b, const int32_t *lb,     \
+                            int32_t n, NAME##_vec *V, int32_t *out)                                       \
+    {                                                                                                     \
+        int32_t j, w, l, maxlen = 0;                                                                      \
+        const NAME##_vec ones = ~(NAME##_vec){0};                                                         \
+        for (l = 0; l < n; ++l) if (lb[l] > maxlen) maxlen = lb[l];                                       \
+        for (w = 0; w < W; ++w) V[w] = ones;                                                              \
+        for (j = 0; j < maxlen; ++j) {                                                                    \
+            uint32_t sym[N];                                                                              \
+            NAME##_vec carry = (NAME##_vec){0};                                                           \
+            for (l = 0; l < N; ++l) sym[l] = (l < n && j < lb[l]) ? b[l][j] : PAD_SYM;                    \
+            for (w = 0; w < W; ++w) {                                                                     \
+                const uint64_t *row = M + (size_t)w * SYMS;                                               \
+                NAME##_vec mw, u, t, s;                                                                   \
+                for (l = 0; l < N; ++l) mw[l] = row[sym[l]];            /* gather: lane l's symbol */      \
+                u = V[w] & mw;                                                                            \
+                t = V[w] + u;                                                                             \
+                s = t - carry;                                          /* carry is a 0 / -1 lane mask */  \
+                carry = (NAME##_vec)(t < u) | (NAME##_vec)(s < t);                                        \
+                V[w] = s | (V[w] & ~mw);                                                                  \
+            }                                                                                             \
+        }                                                                                                 \
+        for (l = 0; l < n; ++l) {                                                                         \
+            int32_t lcs = 0;                                                                              \
+            for (w = 0; w < W; ++w) lcs += __builtin_popcountll(~V[w][l]);                                \
+            out[l] = lcs;                                                                                 \
+        }                                                                                                 \
+    }
+
+DEFINE_LCS_VEC(lcs_v2, 2, )
+DEFINE_LCS_VEC(lcs_v4, 4, )
+DEFINE_LCS_VEC(lcs_v8, 8, )
+#if defined(__x86_64__)
+DEFINE_LCS_VEC(lcs_v4_avx2, 4, __attribute__((target("avx2"))))
+DEFINE_LCS_VEC(lcs_v8_avx512, 8, __attribute__((target("avx512f,avx512bw,avx512dq,avx512vl"))))
+#endif
+
+/* ISA codes of bitpar_rowsets: 0 scalar; 2 / 4 / 8 generic vectors of that many lanes (compiled for the
+ * baseline ISA: the code path of the wide variants on any host); 14 = AVX2 (a = 4); 18 = AVX-512 (a = 8);
+ * -1 = the widest the host supports natively. */
+int bitpar_best_isa(void)
+{
+#if defined(__x86_64__)
+    __builtin_cpu_init();
+    if (__builtin_cpu_supports("avx512f") && __builtin_cpu_supports("avx512bw") &&
+        __builtin_cpu_supports("avx512dq") && __builtin_cpu_supports("avx512vl")) return 18;
+    if (__builtin_cpu_supports("avx2")) return 14;
+#endif
+    return 2;
+}
+
+static int isa_lanes(int isa) { return isa == 0 ? 1 : (isa == 14 ? 4 : (isa == 18 ? 8 : isa)); }
+
 typedef struct {
-    const uint8_t *codes; const int64_t *offsets; const int64_t *pi, *pj; int64_t n;
-    int32_t *out; int64_t *next; pthread_mutex_t *mu; int32_t max_len;
+    const uint8_t *codes; const int64_t *offsets;
+    const int64_t *row_i, *col_ptr, *col_j; int64_t n_rows;
+    int32_t *out; int64_t *next; pthread_mutex_t *mu; int32_t max_len; int isa;
 } bp_job;
 
 static void *bp_worker(void *arg)
 {
     bp_job *jb = (bp_job *)arg;
-    int32_t W = (jb->max_len + 63) / 64;
-    uint64_t *M = (uint64_t *)malloc(sizeof(uint64_t) * SYMS * (size_t)(W + 1));
-    uint64_t *V = (uint64_t *)malloc(sizeof(uint64_t) * (size_t)(W + 1));
+    const int32_t Wmax = (jb->max_len + 63) / 64;
+    const int lanes = isa_lanes(jb->isa);
+    uint64_t *M = NULL, *V = NULL;
+    if (posix_memalign((void **)&M, 64, sizeof(uint64_t) * SYMS * (size_t)(Wmax + 1)) != 0) return NULL;
+    if (posix_memalign((void **)&V, 64, sizeof(uint64_t) * 8 * (size_t)(Wmax + 1)) != 0) { free(M); return NULL; }
     for (;;) {
-        int64_t p0, p1, p;
+        int64_t r, c;
         pthread_mutex_lock(jb->mu);
-        p0 = *jb->next; *jb->next = p0 + 256;
+        r = *jb->next; *jb->next = r + 1;
         pthread_mutex_unlock(jb->mu);
-        if (p0 >= jb->n) break;
-        p1 = p0 + 256 < jb->n ? p0 + 256 : jb->n;
-        for (p = p0; p < p1; ++p) {
-            int64_t i = jb->pi[p], j = jb->pj[p];
-            int32_t li = (int32_t)(jb->offsets[i + 1] - jb->offsets[i]);
-            int32_t lj = (int32_t)(jb->offsets[j + 1] - jb->offsets[j]);
-            const uint8_t *si = jb->codes + jb->offsets[i], *sj = jb->codes + jb->offsets[j];
-            jb->out[p] = li <= lj ? bitpar_lcs(si, li, sj, lj, M, V) : bitpar_lcs(sj, lj, si, li, M, V);
+        if (r >= jb->n_rows) break;
+        {
+            const int64_t i = jb->row_i[r];
+            const uint8_t *a = jb->codes + jb->offsets[i];
+            const int32_t la = (int32_t)(jb->offsets[i + 1] - jb->offsets[i]);
+            const int32_t W = (la + 63) / 64;
+            build_table(a, la, W, M);                    /* once per row: shared by all its columns */
+            for (c = jb->col_ptr[r]; c < jb->col_ptr[r + 1]; c += lanes) {
+                const uint8_t *b[8]; int32_t lb[8]; int32_t n = 0, l;
+                for (l = 0; l < lanes && c + l < jb->col_ptr[r + 1]; ++l, ++n) {
+                    const int64_t j = jb->col_j[c + l];
+                    b[l] = jb->codes + jb->offsets[j];
+                    lb[l] = (int32_t)(jb->offsets[j + 1] - jb->offsets[j]);
+                }
+                switch (jb->isa) {
+                case 0:  jb->out[c] = lcs_scalar(M, W, b[0], lb[0], V); break;
+                case 2:  lcs_v2(M, W, b, lb, n, (lcs_v2_vec *)V, jb->out + c); break;
+                case 4:  lcs_v4(M, W, b, lb, n, (lcs_v4_vec *)V, jb->out + c); break;
+                case 8:  lcs_v8(M, W, b, lb, n, (lcs_v8_vec *)V, jb->out + c); break;
+#if defined(__x86_64__)
+                case 14: lcs_v4_avx2(M, W, b, lb, n, (lcs_v4_avx2_vec *)V, jb->out + c); break;
+                case 18: lcs_v8_avx512(M, W, b, lb, n, (lcs_v8_avx512_vec *)V, jb->out + c); break;
+#endif
+                default: break;
+                }
+            }
         }
     }
     free(M); free(V);
     return NULL;
 }
 
-/* codes must already be encoded (< 32).  max_len = the longest sequence among the pairs. */
-int bitpar_pairs(const uint8_t *codes, const int64_t *offsets, const int64_t *pi, const int64_t *pj,
-                 int64_t n, int32_t max_len, int32_t *lcs_out, int32_t n_threads)
+/*
+ * LCS of row sequence row_i[r] against each of col_j[col_ptr[r] .. col_ptr[r+1]) (ORIGINAL indices, codes
+ * already encoded, < 25), r = 0..n_rows-1; lcs_out is parallel to col_j.  The row carries the bit-vectors
+ * whatever the lengths (LCS is symmetric).  Returns 0, or -1 for an ISA the host cannot run.
+ */
+int bitpar_rowsets(const uint8_t *codes, const int64_t *offsets, const int64_t *row_i, const int64_t *col_ptr,
+                   const int64_t *col_j, int64_t n_rows, int32_t max_len, int32_t *lcs_out, int32_t n_threads, int isa)
 {
     pthread_t th[256];
     pthread_mutex_t mu = PTHREAD_MUTEX_INITIALIZER;
     int64_t next = 0;
     bp_job jb;
-    int t;
+    int t, best = bitpar_best_isa();
+    if (isa < 0) isa = best;
+    if (isa != 0 && isa != 2 && isa != 4 && isa != 8 && isa != 14 && isa != 18) return -1;
+    if ((isa == 14 && best != 14 && best != 18) || (isa == 18 && best != 18)) return -1;
     if (n_threads < 1) n_threads = 1;
     if (n_threads > 256) n_threads = 256;
-    jb.codes = codes; jb.offsets = offsets; jb.pi = pi; jb.pj = pj; jb.n = n; jb.out = lcs_out;
-    jb.next = &next; jb.mu = &mu; jb.max_len = max_len;
+    jb.codes = codes; jb.offsets = offsets; jb.row_i = row_i; jb.col_ptr = col_ptr; jb.col_j = col_j;
+    jb.n_rows = n_rows; jb.out = lcs_out; jb.next = &next; jb.mu = &mu; jb.max_len = max_len; jb.isa = isa;
     for (t = 0; t < n_threads; ++t)
         if (pthread_create(&th[t], NULL, bp_worker, &jb) != 0) { n_threads = t; break; }
     if (n_threads == 0) bp_worker(&jb);

@@ -41,9 +41,11 @@ def _load():
         lib.oracle_pairs.argtypes = [u8p, i64p, i64p, i64p, ctypes.c_int64,
                                      ctypes.POINTER(ctypes.c_int32),
                                      ctypes.POINTER(ctypes.c_double), ctypes.c_int32]
-        lib.bitpar_pairs.restype = ctypes.c_int
-        lib.bitpar_pairs.argtypes = [u8p, i64p, i64p, i64p, ctypes.c_int64, ctypes.c_int32,
-                                     ctypes.POINTER(ctypes.c_int32), ctypes.c_int32]
+        lib.bitpar_rowsets.restype = ctypes.c_int
+        lib.bitpar_rowsets.argtypes = [u8p, i64p, i64p, i64p, i64p, ctypes.c_int64, ctypes.c_int32,
+                                       ctypes.POINTER(ctypes.c_int32), ctypes.c_int32, ctypes.c_int]
+        lib.bitpar_best_isa.restype = ctypes.c_int
+        lib.bitpar_best_isa.argtypes = []
         _lib = lib
     return _lib
 
@@ -138,17 +140,44 @@ def rows(seqs, offsets, i0, i1, want_sim=True, n_threads=None):
     return pairs(seqs, offsets, perm[ii], perm[jj], want_sim, n_threads)
 
 
-def bitpar_pairs(seqs, offsets, pi, pj, n_threads=None):
-    """CONTEXT BASELINE, not an oracle: the paper's own CPU design (64-bit bit-parallel LCS, one pair
-    per task over threads; oracle/bitpar_cpu.c).  LCS (int32) for pairs in ORIGINAL index space."""
+BITPAR_ISA_NAMES = {0: "scalar (1 pair per step)", 2: "generic 128-bit vectors (a = 2)", 4: "generic 256-bit vectors (a = 4)",
+                    8: "generic 512-bit vectors (a = 8)", 14: "AVX2 (a = 4)", 18: "AVX-512 (a = 8)"}
+
+
+def bitpar_best_isa():
+    """The widest multi-pair variant of oracle/bitpar_cpu.c this host runs natively (an ISA code)."""
+    return int(_load().bitpar_best_isa())
+
+
+def bitpar_rowsets(seqs, offsets, row_i, col_ptr, col_j, isa=-1, n_threads=None):
+    """CONTEXT BASELINE, not an oracle: the paper's own CPU design (oracle/bitpar_cpu.c):
+    64-bit bit-parallel LCS, one task per row sequence (match table built once), its columns taken `a` per
+    SIMD register, tasks over threads.  Row r = sequence row_i[r] against col_j[col_ptr[r]:col_ptr[r+1]]
+    (ORIGINAL indices).  Returns LCS (int32) parallel to col_j."""
     codes, cp = _u8(encode(seqs))
     offsets, op = _i64(offsets)
-    pi, pip = _i64(pi)
-    pj, pjp = _i64(pj)
-    lcs = np.empty(pi.size, dtype=np.int32)
+    row_i, rp = _i64(row_i)
+    col_ptr, pp = _i64(col_ptr)
+    col_j, jp = _i64(col_j)
+    lcs = np.empty(col_j.size, dtype=np.int32)
     if n_threads is None:
         n_threads = n_threads_default()
     max_len = int(np.diff(offsets).max()) if offsets.size > 1 else 0
-    _load().bitpar_pairs(cp, op, pip, pjp, pi.size, max_len,
-                         lcs.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), int(n_threads))
+    rc = _load().bitpar_rowsets(cp, op, rp, pp, jp, row_i.size, max_len,
+                                lcs.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), int(n_threads), int(isa))
+    if rc != 0:
+        raise ValueError("bitpar_rowsets: ISA code %d is not supported on this host" % isa)
     return lcs
+
+
+def bitpar_pairs(seqs, offsets, pi, pj, isa=-1, n_threads=None):
+    """bitpar_rowsets for a flat pair list (ORIGINAL index space): pairs are grouped by pi, which carries
+    the bit-vectors.  LCS (int32) in the order of the input pairs."""
+    pi = np.asarray(pi, dtype=np.int64)
+    pj = np.asarray(pj, dtype=np.int64)
+    order = np.argsort(pi, kind="stable")
+    rows, counts = np.unique(pi[order], return_counts=True)
+    col_ptr = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    out = np.empty(pi.size, dtype=np.int32)
+    out[order] = bitpar_rowsets(seqs, offsets, rows, col_ptr, pj[order], isa, n_threads)
+    return out

@@ -86,3 +86,45 @@ def cut(merges, k, threshold):
         roots.setdefault(r, leaf)
         labels[leaf] = roots[r]
     return labels
+
+
+def dendrogram_pair_heights(k, id_a, id_b, sim, qi, qj):
+    """For leaf pairs (qi[q], qj[q]), qi != qj: the merge similarity at which the two leaves first share a
+    cluster, i.e. the similarity of their lowest common ancestor in the dendrogram given as k-1 merges
+    (merge t joins clusters id_a[t], id_b[t] into cluster k + t; scipy ids).  For a single-linkage dendrogram
+    this is the bottleneck (smallest edge) of the path between the leaves in the spanning tree it came from,
+    which is what the cycle property of a maximum spanning tree bounds: similarity(i, j) <= height(i, j) for
+    EVERY pair.  Plain binary lifting over the 2k-1 nodes, vectorised over the queries; any k.
+    Pinned in tests/test_slink_pins.py against replaying the merges one by one."""
+    k = int(k)
+    n = 2 * k - 1
+    id_a = np.asarray(id_a, dtype=np.int64)
+    id_b = np.asarray(id_b, dtype=np.int64)
+    sim = np.asarray(sim, dtype=np.float64)
+    parent = np.arange(n, dtype=np.int64)                     # the root is its own parent
+    parent[id_a] = k + np.arange(k - 1)
+    parent[id_b] = k + np.arange(k - 1)
+    depth = np.zeros(n, dtype=np.int64)
+    dl, pl = depth.tolist(), parent.tolist()
+    for v in range(n - 2, -1, -1):                            # a parent's id is larger than its children's
+        dl[v] = dl[pl[v]] + 1
+    depth = np.asarray(dl, dtype=np.int64)
+    levels = max(1, int(depth.max()).bit_length())
+    up = [parent]
+    for _ in range(1, levels):
+        up.append(up[-1][up[-1]])
+    a = np.asarray(qi, dtype=np.int64).copy()
+    b = np.asarray(qj, dtype=np.int64).copy()
+    swap = depth[a] < depth[b]
+    a[swap], b[swap] = b[swap], a[swap]                       # a is the deeper one
+    diff = depth[a] - depth[b]
+    for j in range(levels):
+        m = ((diff >> j) & 1).astype(bool)
+        a[m] = up[j][a[m]]
+    for j in range(levels - 1, -1, -1):
+        m = up[j][a] != up[j][b]
+        a[m] = up[j][a[m]]
+        b[m] = up[j][b[m]]
+    lca = np.where(a == b, a, parent[a])
+    assert np.all(lca >= k), "a query pair with qi == qj"
+    return sim[lca - k]

@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <atomic>
+#include <deque>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -44,6 +46,23 @@ inline BlockPlan plan_blocks(uint32_t len, bool force32) {
 
 struct Bucket { int64_t r0, r1; int nblk, wb; };   // rows [r0, r1) share one kernel variant
 
+constexpr uint32_t DEFAULT_ROWS_PER_CTA = 2;       // TA on the register path (famsa_ctx_set_tuning)
+constexpr uint32_t DEFAULT_L2_GROUP_MB  = 24;      // residue-stream slice one column group of a launch re-reads from L2
+
+// Staging of the HOST-output path (famsa_lcs_rows_host*): two device row-chunk buffers, two streams and the
+// events that order them; pooled per process (famsa_sweep.cu).
+struct HostChunkTimers { cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr}; double bytes = 0.0; };   // sweep start/end, copy start/end
+struct Staging {
+    int       device = 0;
+    size_t    pairs = 0;                            // capacity of each buffer, in pairs
+    uint16_t* lcs[2] = {nullptr, nullptr};
+    float*    sim[2] = {nullptr, nullptr};
+    cudaStream_t s_compute = nullptr, s_copy = nullptr;
+    cudaEvent_t  ev_done[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
+    bool      profile = false;                      // famsa_host_profile: time every chunk's sweep and copy
+    std::deque<HostChunkTimers> timers;
+};
+
 }  // namespace famsa
 
 struct famsa_ctx {
@@ -66,20 +85,23 @@ struct famsa_ctx {
     uint32_t* d_len = nullptr;
     uint32_t* d_toff = nullptr;
     uint32_t* d_goff = nullptr;
-    // row-block staging for famsa_lcs_rows_host (lazily allocated)
-    uint16_t* d_lcs_buf[2] = {nullptr, nullptr};
-    float*    d_sim_buf[2] = {nullptr, nullptr};
-    size_t    buf_pairs = 0;
+    // row-block staging of famsa_lcs_rows_host* (acquired lazily from the process-wide pool)
+    famsa::Staging* stg = nullptr;
     int64_t   host_chunks = 0;                  // chunks enqueued by the host path so far
-    cudaStream_t s_compute = nullptr, s_copy = nullptr;
-    cudaEvent_t  ev_done[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
+    bool      host_profile = false;
+    // tuning (famsa_ctx_set_tuning): per ctx, so concurrent calls on other ctxs / streams are unaffected
+    std::atomic<uint32_t> rows_per_cta{famsa::DEFAULT_ROWS_PER_CTA};
+    std::atomic<int>      small_mode{-1};       // -1 auto, 0 never, 1 always: one-warp CTAs, one pair per thread
+    std::atomic<uint32_t> l2_group_mb{famsa::DEFAULT_L2_GROUP_MB};
+    double    pack_ms[4] = {0, 0, 0, 0};        // famsa_pack_profile: H2D + encode, sort, host plan, stream + table build
     std::atomic<int64_t> launches{0};
 };
 
 namespace famsa {
 void set_error(const std::string& msg);
 int  cuda_fail(cudaError_t e, const char* what);          // records text, returns FAMSA_ECUDA
-int  sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim, cudaStream_t st);
+int  sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim, unsigned long long* checksum, cudaStream_t st);
+void staging_release(Staging* s);                          // back to the pool (drains its streams first)
 }  // namespace famsa
 
 #define FAMSA_CUDA(call)                                                     \

@@ -4,6 +4,7 @@
 #include <cub/device/device_radix_sort.cuh>
 
 #include <algorithm>
+#include <chrono>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -128,15 +129,9 @@ using namespace famsa;
 extern "C" void famsa_free(famsa_ctx* ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
+    if (ctx->stg) famsa::staging_release(ctx->stg);       // drains the host path's streams, then back to the pool
     cudaFree(ctx->d_stream); cudaFree(ctx->d_tables); cudaFree(ctx->d_len);
     cudaFree(ctx->d_toff); cudaFree(ctx->d_goff);
-    for (int b = 0; b < 2; ++b) {
-        cudaFree(ctx->d_lcs_buf[b]); cudaFree(ctx->d_sim_buf[b]);
-        if (ctx->ev_done[b]) cudaEventDestroy(ctx->ev_done[b]);
-        if (ctx->ev_copied[b]) cudaEventDestroy(ctx->ev_copied[b]);
-    }
-    if (ctx->s_compute) cudaStreamDestroy(ctx->s_compute);
-    if (ctx->s_copy) cudaStreamDestroy(ctx->s_copy);
     delete ctx;
 }
 
@@ -158,7 +153,7 @@ extern "C" int famsa_pack(const uint8_t* seqs, const int64_t* offsets, int64_t k
             return FAMSA_ELENGTH;
         }
     }
-    if (k > 0xFFFFFFF0LL) { set_error("famsa_pack: k too large"); return FAMSA_EINVAL; }
+    if (k > 0x7FFFFFF0LL) { set_error("famsa_pack: k too large (at most 2^31 - 16 sequences)"); return FAMSA_EINVAL; }
     famsa_ctx* ctx = new (std::nothrow) famsa_ctx();
     if (!ctx) { set_error("famsa_pack: host allocation failed"); return FAMSA_ENOMEM; }
     int rc;
@@ -212,6 +207,9 @@ static int pack_impl(const uint8_t* seqs, const int64_t* offsets, int64_t k, int
     ctx->device = device; ctx->sm_count = prop.multiProcessorCount; ctx->k = k;
     ctx->n_groups = (k + GROUP - 1) / GROUP;
     const int64_t total = offsets[k];
+    using clk = std::chrono::steady_clock;
+    auto ms_since = [](clk::time_point t) { return std::chrono::duration<double, std::milli>(clk::now() - t).count(); };
+    clk::time_point t_phase = clk::now();
     DevTmp tmp;
     cudaStream_t st = nullptr;           // legacy default stream; pack synchronises before returning
 
@@ -237,6 +235,7 @@ static int pack_impl(const uint8_t* seqs, const int64_t* offsets, int64_t k, int
                   " is neither a residue code (< 25) nor an amino-acid letter");
         return FAMSA_ESYMBOL;
     }
+    ctx->pack_ms[0] = ms_since(t_phase); t_phase = clk::now();
 
     // ---- a2 length sort (descending, stable)
     uint32_t *d_key = nullptr, *d_key2 = nullptr, *d_idx = nullptr, *d_perm = nullptr;
@@ -260,6 +259,7 @@ static int pack_impl(const uint8_t* seqs, const int64_t* offsets, int64_t k, int
     }
     ctx->max_len = k ? ctx->len[0] : 0;
     ctx->large_cw = ctx->max_len > (uint32_t)CW_SMALL * 32;
+    ctx->pack_ms[1] = ms_since(t_phase); t_phase = clk::now();
 
     // ---- host plan: table offsets, block plans, buckets, group offsets, length prefix sums
     ctx->toff.resize(k); ctx->goff.resize(ctx->n_groups + 1); ctx->len_prefix.resize(k + 1);
@@ -288,6 +288,8 @@ static int pack_impl(const uint8_t* seqs, const int64_t* offsets, int64_t k, int
     ctx->stream_bytes = (size_t)chunks_total * GROUP * CHUNK;
     ctx->table_bytes = (size_t)rows_total * ROW_BYTES;
 
+    ctx->pack_ms[2] = ms_since(t_phase); t_phase = clk::now();
+
     // ---- device-resident set
     uint32_t* d_twords = nullptr;
     FAMSA_TRY(tmp.alloc(&d_twords, twords.size()));
@@ -310,6 +312,13 @@ static int pack_impl(const uint8_t* seqs, const int64_t* offsets, int64_t k, int
     }
     FAMSA_CUDA(cudaGetLastError());
     FAMSA_CUDA(cudaStreamSynchronize(st));
+    ctx->pack_ms[3] = ms_since(t_phase);
+    return FAMSA_OK;
+}
+
+extern "C" int famsa_pack_profile(const famsa_ctx* ctx, double* ms4) {
+    if (!ctx || !ms4) { set_error("famsa_pack_profile: null argument"); return FAMSA_EINVAL; }
+    for (int q = 0; q < 4; ++q) ms4[q] = ctx->pack_ms[q];
     return FAMSA_OK;
 }
 

@@ -35,7 +35,26 @@ struct SweepArgs {
     uint32_t        ta;          // rows per CTA
     uint32_t        n_col_tiles;
     uint32_t        nblk;        // table blocks per row (1 on the register path)
+    uint32_t        row_tiles;   // row tiles of this launch
+    uint32_t        cg_tiles;    // column tiles per column group (L2 blocking of the residue stream, see tile_coords)
+    unsigned long long* checksum;   // DEVICE u64[2] or nullptr: += sum of LCS, += sum of similarity bit patterns
 };
+
+// CTA -> (row tile, column tile).  The grid is walked column GROUP by column group: inside a group of
+// cg_tiles column tiles every row tile of the launch is swept before the next group starts, so the slice
+// of the residue stream in use (cg_tiles x 128 sequences, sized to ~24 MB by the host) is re-read from L2
+// by each of the launch's row tiles instead of the whole 129 MB stream cycling through the 126 MB L2 once
+// per row tile (r01: 22 GB of DRAM reads for a launch whose algorithmic traffic is 1.6 GB).
+// Columns ascend inside and across groups, so the longest sequences are still scheduled first.
+__device__ __forceinline__ void tile_coords(const SweepArgs& a, uint32_t& row_tile, uint32_t& col_tile) {
+    const uint32_t per_group = a.row_tiles * a.cg_tiles;
+    const uint32_t cg = blockIdx.x / per_group;
+    const uint32_t rem = blockIdx.x - cg * per_group;
+    const uint32_t c0 = cg * a.cg_tiles;
+    const uint32_t gc = min(a.cg_tiles, a.n_col_tiles - c0);        // the last group may be narrower
+    row_tile = rem / gc;
+    col_tile = c0 + rem % gc;
+}
 
 // ---- table staging: one TMA bulk copy (cp.async.bulk, global -> shared) per tile, completion on an
 // mbarrier; no registers or LSU instructions are spent on it and the waiting warps sleep on the barrier.
@@ -140,36 +159,39 @@ __device__ __forceinline__ void sweep_block(uint32_t (&V)[W], const uint4* __res
     }
 }
 
-__device__ __forceinline__ void store_pair(const SweepArgs& a, uint32_t i, uint32_t j, uint32_t la, uint32_t lb, uint32_t lcs) {
-    int64_t pos = (int64_t)i * (i - 1) / 2 - a.out_base + j;
-    if (a.lcs_out) a.lcs_out[pos] = (unsigned short)lcs;
-    if (a.sim_out) {
-        // indel = |A| + |B| - 2 LCS; similarity = LCS / indel^2
-        unsigned long long indel = (unsigned long long)la + lb - 2ull * lcs;
-        a.sim_out[pos] = __fdiv_rn(__uint2float_rn(lcs), __ull2float_rn(indel * indel));
+// Epilogue (a6, a7) for one row of a warp: indel = |A| + |B| - 2 LCS, similarity = LCS / indel^2
+// (PAPER.md:42), stored with the streaming hint (st.global.cs: written once, never re-read by the sweep, so
+// the lines should not displace the residue stream in L2).  Called by ALL lanes of the warp (`valid` says
+// which lanes own an entry) so that the optional checksum can use warp reductions.
+__device__ __forceinline__ void store_pair(const SweepArgs& a, bool valid, uint32_t i, uint32_t j, uint32_t la, uint32_t lb, uint32_t lcs) {
+    const int64_t pos = (int64_t)i * (i - 1) / 2 - a.out_base + j;
+    uint32_t sim_bits = 0;
+    if (valid) {
+        if (a.lcs_out) __stcs(a.lcs_out + pos, (unsigned short)lcs);
+        if (a.sim_out) {
+            const unsigned long long indel = (unsigned long long)la + lb - 2ull * lcs;
+            const float sim = __fdiv_rn(__uint2float_rn(lcs), __ull2float_rn(indel * indel));
+            __stcs(a.sim_out + pos, sim);
+            sim_bits = __float_as_uint(sim);
+        }
+    }
+    if (a.checksum) {                                       // kernel-uniform
+        const uint32_t sl = __reduce_add_sync(0xffffffffu, valid ? lcs : 0u);          // <= 32 x 65535
+        const uint32_t s_lo = __reduce_add_sync(0xffffffffu, sim_bits & 0xFFFFu);
+        const uint32_t s_hi = __reduce_add_sync(0xffffffffu, sim_bits >> 16);
+        if ((threadIdx.x & 31) == 0) {
+            if (sl) atomicAdd(a.checksum, (unsigned long long)sl);
+            if (s_lo | s_hi) atomicAdd(a.checksum + 1, ((unsigned long long)s_hi << 16) + s_lo);
+        }
     }
 }
 
 // ---- register path: every row of the launch fits one block of W words --------------------------
-// Two rows per thread at once (NR = 2) while 2W words of V fit comfortably in registers: both rows
-// see the same residue, so the address PRMT and the residue-stream loads are shared and the two
-// carry chains are independent (more ILP per warp).
-#ifndef FAMSA_NR_POLICY
-#define FAMSA_NR_POLICY 2
-#endif
-__host__ __device__ constexpr int rows_per_thread(int w) {
-#if FAMSA_NR_POLICY == 0
-    return w <= 16 ? 2 : 1;
-#elif FAMSA_NR_POLICY == 1
-    return w <= 6 ? 4 : (w <= 10 ? 3 : (w <= 16 ? 2 : 1));
-#elif FAMSA_NR_POLICY == 2
-    return w <= 8 ? 3 : (w <= 16 ? 2 : 1);
-#elif FAMSA_NR_POLICY == 3
-    return w <= 4 ? 4 : (w <= 7 ? 3 : (w <= 20 ? 2 : 1));
-#else
-    return 1;
-#endif
-}
+// NR rows per thread at once (3 for W <= 8, 2 for W <= 16, else 1) while NR x W words of V fit
+// comfortably in registers: the rows see the same residue, so the address PRMT and the residue-stream
+// loads are shared and the NR carry chains are independent (more ILP per warp).  Small jobs (too few
+// pairs to fill the SMs' warp slots) use NR = 1 and one-warp CTAs instead: see sweep_rows().
+__host__ __device__ constexpr int rows_per_thread(int w) { return w <= 8 ? 3 : (w <= 16 ? 2 : 1); }
 
 template <int W, int NR, int TS>
 __device__ __forceinline__ void residue_step_rows(uint32_t (&V)[NR][W], uint32_t addr) {
@@ -217,17 +239,24 @@ __device__ __forceinline__ void sweep_rows_block(uint32_t (&V)[NR][W], const uin
         word_step_rows<W, NR, TS>(V, q == 0 ? cur.x : (q == 1 ? cur.y : cur.z), tbase);
 }
 
-template <int W>
+// Every working warp ends with griddepcontrol.wait: launches after the first one of a call are
+// programmatic dependents (they start while their predecessor drains), and a grid whose CTAs wait for the
+// predecessor's completion cannot itself complete earlier -- so "the last launch of the call is done"
+// implies "every launch of the call is done", which is what an event recorded after the call relies on.
+// (Without the launch attribute the instruction is a no-op.)
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <int W, int NR>
 __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
     extern __shared__ __align__(256) uint8_t smem[];
     asm volatile("griddepcontrol.launch_dependents;");
     constexpr int WST = (W + 1) & ~1;
     constexpr int TS = WST * ROW_BYTES;                  // bytes between the tables of consecutive rows
-    constexpr int NR = rows_per_thread(W);
-    const uint32_t col_tile = blockIdx.x % a.n_col_tiles, row_tile = blockIdx.x / a.n_col_tiles;
+    uint32_t row_tile, col_tile;
+    tile_coords(a, row_tile, col_tile);
     const uint32_t r_lo = a.r0 + row_tile * a.ta;
     const uint32_t r_hi = min(r_lo + a.ta, a.r1);
-    const uint32_t j0 = col_tile * TB;
+    const uint32_t j0 = col_tile * blockDim.x;           // blockDim.x = 128 columns, or 32 for small jobs
     if (j0 + 1 >= r_hi) return;                          // whole tile on or above the diagonal
     // stage the tile's tables: rows r_lo..r_hi-1 are contiguous (same stride each).  With NR > 1 the
     // last step of a warp may run past row r_hi-1: the launch allocates NR-1 extra table slots, whose
@@ -259,10 +288,11 @@ __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
             uint32_t lcs = 0;
 #pragma unroll
             for (int w = 0; w < W; ++w) lcs += __popc(~V[p][w]);
-            const uint32_t row = i + p;
-            if (row < r_hi && j < row) store_pair(a, row, j, a.len[row], lb, lcs);
+            const uint32_t row = i + p;                  // warp-uniform
+            if (row < r_hi) store_pair(a, j < row, row, j, a.len[row], lb, lcs);
         }
     }
+    pdl_wait();
 }
 
 // ---- blocked path: rows of nblk blocks x W words; one row per CTA; carry bit-vector per thread --
@@ -271,7 +301,8 @@ __global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
     extern __shared__ __align__(256) uint8_t smem[];
     asm volatile("griddepcontrol.launch_dependents;");
     constexpr int WST = (W + 1) & ~1;
-    const uint32_t col_tile = blockIdx.x % a.n_col_tiles, row_tile = blockIdx.x / a.n_col_tiles;
+    uint32_t row_tile, col_tile;
+    tile_coords(a, row_tile, col_tile);
     const uint32_t i = a.r0 + row_tile;
     const uint32_t j0 = col_tile * TB;
     if (j0 >= i) return;
@@ -301,7 +332,10 @@ __global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
             for (int w = 0; w < W; ++w) lcs += __popc(~V[w]);
         }
     }
-    if (active && j < i) store_pair(a, i, j, a.len[i], a.len[j], lcs);
+    if (active) {
+        store_pair(a, j < i, i, j, a.len[i], j < i ? a.len[j] : 0, lcs);
+        pdl_wait();
+    }
 }
 
 }  // namespace famsa
@@ -312,28 +346,22 @@ namespace famsa {
 // Launches after the first one of a famsa_lcs_rows call carry the programmatic-stream-serialization
 // attribute: the launches of one call read the same read-only set and write disjoint output ranges,
 // so the next bucket's CTAs may fill the SMs while the previous launch drains its last wave
-// (every sweep kernel executes griddepcontrol.launch_dependents on entry; none needs .wait).
+// (every sweep kernel executes griddepcontrol.launch_dependents on entry and griddepcontrol.wait at
+// the end of each working warp, see pdl_wait()).
 template <typename K>
-static cudaError_t launch_sweep(K kernel, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st, bool overlap) {
+static cudaError_t launch_sweep(K kernel, const SweepArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t st, bool overlap) {
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(TB); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = overlap ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kernel, a);
 }
-template <int W>
-static cudaError_t launch_short(const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st, bool overlap) {
-    return launch_sweep(sweep_short_kernel<W>, a, grid, smem, st, overlap);
-}
-template <int W, int CW>
-static cudaError_t launch_long(const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st, bool overlap) {
-    return launch_sweep(sweep_long_kernel<W, CW>, a, grid, smem, st, overlap);
-}
 
-#define SHORT_CASE(W) case W: return launch_short<W>(a, grid, smem, st, overlap);
-static cudaError_t dispatch_short(int w, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st, bool overlap) {
+#define SHORT_CASE(W) case W: return small ? launch_sweep(sweep_short_kernel<W, 1>, a, grid, block, smem, st, overlap) \
+                                           : launch_sweep(sweep_short_kernel<W, rows_per_thread(W)>, a, grid, block, smem, st, overlap);
+static cudaError_t dispatch_short(int w, bool small, const SweepArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t st, bool overlap) {
     switch (w) {
         SHORT_CASE(1) SHORT_CASE(2) SHORT_CASE(3) SHORT_CASE(4) SHORT_CASE(5) SHORT_CASE(6) SHORT_CASE(7) SHORT_CASE(8)
         SHORT_CASE(9) SHORT_CASE(10) SHORT_CASE(11) SHORT_CASE(12) SHORT_CASE(13) SHORT_CASE(14) SHORT_CASE(15) SHORT_CASE(16)
@@ -342,9 +370,9 @@ static cudaError_t dispatch_short(int w, const SweepArgs& a, unsigned grid, size
         default: return cudaErrorInvalidValue;
     }
 }
-#define LONG_CASE(W) case W: return launch_long<W, CW_SMALL>(a, grid, smem, st, overlap);
+#define LONG_CASE(W) case W: return launch_sweep(sweep_long_kernel<W, CW_SMALL>, a, grid, TB, smem, st, overlap);
 static cudaError_t dispatch_long(int w, bool large, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st, bool overlap) {
-    if (large) return w == 32 ? launch_long<32, CW_LARGE>(a, grid, smem, st, overlap) : cudaErrorInvalidValue;
+    if (large) return w == 32 ? launch_sweep(sweep_long_kernel<32, CW_LARGE>, a, grid, TB, smem, st, overlap) : cudaErrorInvalidValue;
     switch (w) {
         LONG_CASE(17) LONG_CASE(18) LONG_CASE(19) LONG_CASE(20) LONG_CASE(21) LONG_CASE(22) LONG_CASE(23) LONG_CASE(24)
         LONG_CASE(25) LONG_CASE(26) LONG_CASE(27) LONG_CASE(28) LONG_CASE(29) LONG_CASE(30) LONG_CASE(31) LONG_CASE(32)
@@ -352,9 +380,16 @@ static cudaError_t dispatch_long(int w, bool large, const SweepArgs& a, unsigned
     }
 }
 
-static uint32_t g_rows_per_cta = 2;     // TA; tunable through famsa_set_tuning (tests sweep it)
+// Column tiles per column group, so that one group's slice of the residue stream is ~l2_group_bytes.
+static uint32_t column_group_tiles(const famsa_ctx* ctx, uint32_t r1, uint32_t n_col_tiles, double l2_group_bytes) {
+    const int64_t g_end = std::min<int64_t>(((int64_t)r1 - 1 + GROUP - 1) / GROUP, ctx->n_groups);
+    const double bytes = (double)ctx->goff[g_end] * (GROUP * CHUNK);          // stream bytes of columns [0, r1-1)
+    const double per_tile = std::max(bytes / std::max<uint32_t>(n_col_tiles, 1), 1.0);
+    const double t = l2_group_bytes / per_tile;
+    return (uint32_t)std::min<double>(std::max(t, 1.0), (double)std::max<uint32_t>(n_col_tiles, 1));
+}
 
-int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim, cudaStream_t st) {
+int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim, unsigned long long* checksum, cudaStream_t st) {
     SweepArgs a;
     a.stream = reinterpret_cast<const uint4*>(ctx->d_stream);
     a.goff = ctx->d_goff;
@@ -362,25 +397,39 @@ int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim
     a.toff = ctx->d_toff;
     a.len = ctx->d_len;
     a.lcs_out = lcs; a.sim_out = sim;
+    a.checksum = checksum;
     a.out_base = i0 * (i0 - 1) / 2;
+    const uint32_t rows_per_cta = ctx->rows_per_cta.load();
+    const int small_mode = ctx->small_mode.load();
+    const double l2_group_bytes = (double)ctx->l2_group_mb.load() * 1048576.0;
+    // Small job: too few pairs to give every SM sub-partition a handful of warps at 2-3 rows per thread.
+    // Then every pair gets its own thread (NR = 1, one row per CTA) in one-warp CTAs, so the hardware
+    // scheduler balances the job over the SMs at warp granularity (configs[0]: 124 750 pairs = 3 898 warps
+    // over 592 sub-partitions) instead of a few fat 128-thread CTAs per SM.
+    const bool small = small_mode == 1 || (small_mode < 0 && famsa_rows_pairs(i0, i1) < (int64_t)2048 * ctx->sm_count);
+    const unsigned block = small ? 32 : TB;
     int n_launched = 0;
     for (const Bucket& b : ctx->buckets) {
         int64_t lo = std::max(b.r0, std::max<int64_t>(i0, 1)), hi = std::min(b.r1, i1);   // row 0 is empty
         for (int64_t r = lo; r < hi; r += MAX_ROWS_PER_LAUNCH) {
             a.r0 = (uint32_t)r; a.r1 = (uint32_t)std::min<int64_t>(r + MAX_ROWS_PER_LAUNCH, hi);
             a.nblk = (uint32_t)b.nblk;
-            a.n_col_tiles = (a.r1 - 1 + TB - 1) / TB;                // columns 0 .. r1-2
             const int wst = (b.wb + 1) & ~1;
             cudaError_t e;
             if (b.nblk == 1) {
-                const uint32_t nr = (uint32_t)rows_per_thread(b.wb);
-                a.ta = ((g_rows_per_cta + nr - 1) / nr) * nr;       // a whole number of NR-row steps per CTA
+                a.n_col_tiles = (a.r1 - 1 + block - 1) / block;          // columns 0 .. r1-2
+                const uint32_t nr = small ? 1u : (uint32_t)rows_per_thread(b.wb);
+                a.ta = small ? 1u : ((rows_per_cta + nr - 1) / nr) * nr;   // a whole number of NR-row steps per CTA
                 while (a.ta > nr && (size_t)(a.ta + nr - 1) * wst * ROW_BYTES + 16 > 48 * 1024) a.ta -= nr;   // default dynamic smem limit
-                unsigned row_tiles = (a.r1 - a.r0 + a.ta - 1) / a.ta;
-                e = dispatch_short(b.wb, a, row_tiles * a.n_col_tiles, (size_t)(a.ta + nr - 1) * wst * ROW_BYTES + 16, st, n_launched > 0);
+                a.row_tiles = (a.r1 - a.r0 + a.ta - 1) / a.ta;
+                a.cg_tiles = column_group_tiles(ctx, a.r1, a.n_col_tiles, l2_group_bytes);
+                e = dispatch_short(b.wb, small, a, a.row_tiles * a.n_col_tiles, block, (size_t)(a.ta + nr - 1) * wst * ROW_BYTES + 16, st, n_launched > 0);
             } else {
+                a.n_col_tiles = (a.r1 - 1 + TB - 1) / TB;
                 a.ta = 1;
-                e = dispatch_long(b.wb, ctx->large_cw, a, (a.r1 - a.r0) * a.n_col_tiles, (size_t)wst * ROW_BYTES + 16, st, n_launched > 0);
+                a.row_tiles = a.r1 - a.r0;
+                a.cg_tiles = column_group_tiles(ctx, a.r1, a.n_col_tiles, l2_group_bytes);
+                e = dispatch_long(b.wb, ctx->large_cw, a, a.row_tiles * a.n_col_tiles, (size_t)wst * ROW_BYTES + 16, st, n_launched > 0);
             }
             if (e != cudaSuccess) return cuda_fail(e, "sweep kernel launch");
             ctx->launches++; ++n_launched;
@@ -389,89 +438,185 @@ int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim
     return FAMSA_OK;
 }
 
+// ---- staging sets of the HOST-output path: two device row-chunk buffers, two streams, four events.
+// Pooled per process (idle sets are kept on famsa_free and reused by the next ctx on the same device), so
+// that a caller that packs, sweeps and frees in a loop does not pay cudaMalloc/cudaFree of ~1.6 GB and
+// stream/event creation every time.  famsa_trim() releases the idle sets.
+static std::mutex g_pool_mu;
+static std::vector<Staging*> g_pool;
+
+static void staging_destroy(Staging* s) {
+    if (!s) return;
+    cudaSetDevice(s->device);
+    for (int b = 0; b < 2; ++b) {
+        cudaFree(s->lcs[b]); cudaFree(s->sim[b]);
+        if (s->ev_done[b]) cudaEventDestroy(s->ev_done[b]);
+        if (s->ev_copied[b]) cudaEventDestroy(s->ev_copied[b]);
+    }
+    if (s->s_compute) cudaStreamDestroy(s->s_compute);
+    if (s->s_copy) cudaStreamDestroy(s->s_copy);
+    delete s;
+}
+
+// An idle set of this device with room for `pairs` pairs per buffer, or a new one (idle sets of the device
+// that are too small are released first, so the pool never holds more than it last needed).
+static int staging_acquire(int device, size_t pairs, Staging** out) {
+    *out = nullptr;
+    std::vector<Staging*> drop;
+    Staging* got = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_pool_mu);
+        for (size_t n = 0; n < g_pool.size();) {
+            Staging* s = g_pool[n];
+            if (s->device == device && !got && s->pairs >= pairs) { got = s; g_pool.erase(g_pool.begin() + n); }
+            else if (s->device == device && s->pairs < pairs) { drop.push_back(s); g_pool.erase(g_pool.begin() + n); }
+            else ++n;
+        }
+    }
+    for (Staging* s : drop) staging_destroy(s);
+    if (got) { *out = got; return FAMSA_OK; }
+    Staging* s = new (std::nothrow) Staging();
+    if (!s) { set_error("famsa_lcs_rows_host: host allocation failed"); return FAMSA_ENOMEM; }
+    s->device = device;
+    cudaError_t e = cudaStreamCreateWithFlags(&s->s_compute, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->s_copy, cudaStreamNonBlocking);
+    for (int b = 0; b < 2 && e == cudaSuccess; ++b) {
+        e = cudaEventCreateWithFlags(&s->ev_done[b], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->ev_copied[b], cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) { staging_destroy(s); return cuda_fail(e, "famsa_lcs_rows_host: stream/event creation"); }
+    for (int b = 0; b < 2; ++b) {
+        cudaError_t e1 = cudaMalloc((void**)&s->lcs[b], pairs * sizeof(uint16_t));
+        cudaError_t e2 = cudaMalloc((void**)&s->sim[b], pairs * sizeof(float));
+        if (e1 != cudaSuccess || e2 != cudaSuccess) {
+            cudaGetLastError(); staging_destroy(s);
+            set_error("famsa_lcs_rows_host: device allocation failed"); return FAMSA_ENOMEM;
+        }
+    }
+    s->pairs = pairs;
+    *out = s;
+    return FAMSA_OK;
+}
+
+void staging_release(Staging* s) {                         // called by famsa_free
+    if (!s) return;
+    cudaSetDevice(s->device);
+    cudaStreamSynchronize(s->s_copy); cudaStreamSynchronize(s->s_compute);
+    for (HostChunkTimers& t : s->timers) for (cudaEvent_t e : t.ev) if (e) cudaEventDestroy(e);
+    s->timers.clear(); s->profile = false;
+    std::lock_guard<std::mutex> lk(g_pool_mu);
+    g_pool.push_back(s);
+}
+
 }  // namespace famsa
 
 using namespace famsa;
 
-extern "C" int famsa_set_tuning(int rows_per_cta) {
-    if (rows_per_cta < 1 || rows_per_cta > 12) { set_error("famsa_set_tuning: rows_per_cta must be 1..12"); return FAMSA_EINVAL; }
-    g_rows_per_cta = (uint32_t)rows_per_cta;
+extern "C" int famsa_trim(void) {
+    std::vector<Staging*> all;
+    { std::lock_guard<std::mutex> lk(g_pool_mu); all.swap(g_pool); }
+    for (Staging* s : all) staging_destroy(s);
+    return FAMSA_OK;
+}
+
+extern "C" int famsa_ctx_set_tuning(famsa_ctx* ctx, int rows_per_cta, int small_job_mode, int l2_group_mb) {
+    if (!ctx) { set_error("famsa_ctx_set_tuning: ctx is NULL"); return FAMSA_EINVAL; }
+    if (rows_per_cta < 0 || rows_per_cta > 12) { set_error("famsa_ctx_set_tuning: rows_per_cta must be 0 (default) or 1..12"); return FAMSA_EINVAL; }
+    if (small_job_mode < -1 || small_job_mode > 1) { set_error("famsa_ctx_set_tuning: small_job_mode must be -1 (auto), 0 or 1"); return FAMSA_EINVAL; }
+    if (l2_group_mb < 0 || l2_group_mb > 4096) { set_error("famsa_ctx_set_tuning: l2_group_mb must be 0 (default) or 1..4096"); return FAMSA_EINVAL; }
+    ctx->rows_per_cta.store(rows_per_cta ? (uint32_t)rows_per_cta : DEFAULT_ROWS_PER_CTA);
+    ctx->small_mode.store(small_job_mode);
+    ctx->l2_group_mb.store(l2_group_mb ? (uint32_t)l2_group_mb : DEFAULT_L2_GROUP_MB);
+    return FAMSA_OK;
+}
+
+static int rows_check(famsa_ctx* ctx, int64_t i0, int64_t i1, const void* lcs, const void* sim, const char* who) {
+    if (!ctx) { set_error(std::string(who) + ": ctx is NULL"); return FAMSA_EINVAL; }
+    if (i0 < 0 || i0 > i1 || i1 > ctx->k) { set_error(std::string(who) + ": bad row range"); return FAMSA_ERANGE; }
+    if (!lcs && !sim) { set_error(std::string(who) + ": both outputs are NULL"); return FAMSA_EINVAL; }
     return FAMSA_OK;
 }
 
 extern "C" int famsa_lcs_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_out, float* sim_out,
                               void* cuda_stream) {
-    if (!ctx) { set_error("famsa_lcs_rows: ctx is NULL"); return FAMSA_EINVAL; }
-    if (i0 < 0 || i0 > i1 || i1 > ctx->k) { set_error("famsa_lcs_rows: bad row range"); return FAMSA_ERANGE; }
-    if (!lcs_out && !sim_out) { set_error("famsa_lcs_rows: both outputs are NULL"); return FAMSA_EINVAL; }
+    int rc = rows_check(ctx, i0, i1, lcs_out, sim_out, "famsa_lcs_rows");
+    if (rc != FAMSA_OK) return rc;
     if (famsa_rows_pairs(i0, i1) == 0) return FAMSA_OK;
     FAMSA_CUDA(cudaSetDevice(ctx->device));
-    return sweep_rows(ctx, i0, i1, lcs_out, sim_out, (cudaStream_t)cuda_stream);
+    return sweep_rows(ctx, i0, i1, lcs_out, sim_out, nullptr, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int famsa_lcs_rows_checksum(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_out, float* sim_out,
+                                       uint64_t* checksum_dev, void* cuda_stream) {
+    int rc = rows_check(ctx, i0, i1, lcs_out, sim_out, "famsa_lcs_rows_checksum");
+    if (rc != FAMSA_OK) return rc;
+    if (!checksum_dev) { set_error("famsa_lcs_rows_checksum: checksum_dev is NULL"); return FAMSA_EINVAL; }
+    if (famsa_rows_pairs(i0, i1) == 0) return FAMSA_OK;
+    FAMSA_CUDA(cudaSetDevice(ctx->device));
+    static_assert(sizeof(unsigned long long) == sizeof(uint64_t), "uint64_t");
+    return sweep_rows(ctx, i0, i1, lcs_out, sim_out, reinterpret_cast<unsigned long long*>(checksum_dev), (cudaStream_t)cuda_stream);
 }
 
 static int rows_host_impl(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_host, float* sim_host, bool wait) {
-    if (!ctx) { set_error("famsa_lcs_rows_host: ctx is NULL"); return FAMSA_EINVAL; }
-    if (i0 < 0 || i0 > i1 || i1 > ctx->k) { set_error("famsa_lcs_rows_host: bad row range"); return FAMSA_ERANGE; }
-    if (!lcs_host && !sim_host) { set_error("famsa_lcs_rows_host: both outputs are NULL"); return FAMSA_EINVAL; }
+    int rc = rows_check(ctx, i0, i1, lcs_host, sim_host, "famsa_lcs_rows_host");
+    if (rc != FAMSA_OK) return rc;
     if (famsa_rows_pairs(i0, i1) == 0) return FAMSA_OK;
     FAMSA_CUDA(cudaSetDevice(ctx->device));
-    // lazily create the ping-pong staging (two staging buffers of 1 Mi .. 128 Mi pairs each)
     // chunk size: about 1/8 of the call (so the copy of chunk n overlaps the sweep of chunk n+1),
     // between 1 Mi and 128 Mi pairs, and never smaller than the longest row
     const int64_t total_pairs = famsa_rows_pairs(i0, i1);
     const int64_t chunk_pairs = std::max<int64_t>(std::min<int64_t>(std::max<int64_t>(total_pairs / 8, (int64_t)1 << 20), (int64_t)128 << 20), i1);
     const size_t want = (size_t)std::min<int64_t>(total_pairs, chunk_pairs);
-    if (!ctx->s_compute) {
-        FAMSA_CUDA(cudaStreamCreateWithFlags(&ctx->s_compute, cudaStreamNonBlocking));
-        FAMSA_CUDA(cudaStreamCreateWithFlags(&ctx->s_copy, cudaStreamNonBlocking));
-        for (int b = 0; b < 2; ++b) {
-            FAMSA_CUDA(cudaEventCreateWithFlags(&ctx->ev_done[b], cudaEventDisableTiming));
-            FAMSA_CUDA(cudaEventCreateWithFlags(&ctx->ev_copied[b], cudaEventDisableTiming));
-        }
-    }
-    if (ctx->buf_pairs < want) {
+    if (!ctx->stg || ctx->stg->pairs < want) {
         // size the staging once per ctx (1/8 of the whole triangle, 1 Mi .. 128 Mi pairs, at least one row),
         // so that a stream of growing row-block calls does not reallocate it
         const int64_t tri = ctx->k * (ctx->k - 1) / 2;
         const size_t cap = (size_t)std::max<int64_t>(std::max<int64_t>(std::min<int64_t>(std::max<int64_t>(tri / 8, (int64_t)1 << 20), (int64_t)128 << 20), ctx->k), (int64_t)want);
-        FAMSA_CUDA(cudaDeviceSynchronize());
-        for (int b = 0; b < 2; ++b) {
-            cudaFree(ctx->d_lcs_buf[b]); cudaFree(ctx->d_sim_buf[b]);
-            ctx->d_lcs_buf[b] = nullptr; ctx->d_sim_buf[b] = nullptr;
-        }
-        ctx->buf_pairs = 0;
-        for (int b = 0; b < 2; ++b) {
-            cudaError_t e1 = cudaMalloc((void**)&ctx->d_lcs_buf[b], cap * sizeof(uint16_t));
-            cudaError_t e2 = cudaMalloc((void**)&ctx->d_sim_buf[b], cap * sizeof(float));
-            if (e1 != cudaSuccess || e2 != cudaSuccess) {
-                cudaGetLastError(); set_error("famsa_lcs_rows_host: device allocation failed"); return FAMSA_ENOMEM;
-            }
-        }
-        ctx->buf_pairs = cap;
+        if (ctx->stg) { staging_release(ctx->stg); ctx->stg = nullptr; }       // drains it first
+        rc = staging_acquire(ctx->device, cap, &ctx->stg);
+        if (rc != FAMSA_OK) return rc;
+        ctx->stg->profile = ctx->host_profile;
+        ctx->host_chunks = 0;
     }
-    // chunk the row range so that each chunk fits a buffer (a single row always fits: i < 2^32 / ... k <= buf)
+    Staging* g = ctx->stg;
+    // on any failure below: drain what is already in flight on the two streams, then report
+    auto fail = [&](int code) { cudaStreamSynchronize(g->s_compute); cudaStreamSynchronize(g->s_copy); return code; };
+#define HOST_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return fail(famsa::cuda_fail(e__, #call)); } while (0)
+    // chunk the row range so that each chunk fits a buffer (a single row always fits: cap >= k)
     int64_t r = i0; int64_t done_pairs = 0;
     int64_t& n = ctx->host_chunks;                         // chunks enqueued so far by this ctx: the ping-pong continues across calls
     while (r < i1) {
         int64_t e = r + 1;
         while (e < i1 && famsa_rows_pairs(r, e + 1) <= (int64_t)want) ++e;
         const int64_t np = famsa_rows_pairs(r, e);
-        if (np > (int64_t)ctx->buf_pairs) { set_error("famsa_lcs_rows_host: a single row exceeds the staging buffer"); return FAMSA_ENOMEM; }
+        if (np > (int64_t)g->pairs) { set_error("famsa_lcs_rows_host: a single row exceeds the staging buffer"); return fail(FAMSA_ENOMEM); }
         const int b = (int)(n & 1);
-        if (n >= 2) FAMSA_CUDA(cudaStreamWaitEvent(ctx->s_compute, ctx->ev_copied[b], 0));
-        int rc = sweep_rows(ctx, r, e, lcs_host ? ctx->d_lcs_buf[b] : nullptr, sim_host ? ctx->d_sim_buf[b] : nullptr, ctx->s_compute);
-        if (rc != FAMSA_OK) return rc;
-        FAMSA_CUDA(cudaEventRecord(ctx->ev_done[b], ctx->s_compute));
-        FAMSA_CUDA(cudaStreamWaitEvent(ctx->s_copy, ctx->ev_done[b], 0));
-        if (lcs_host) FAMSA_CUDA(cudaMemcpyAsync(lcs_host + done_pairs, ctx->d_lcs_buf[b], np * sizeof(uint16_t), cudaMemcpyDeviceToHost, ctx->s_copy));
-        if (sim_host) FAMSA_CUDA(cudaMemcpyAsync(sim_host + done_pairs, ctx->d_sim_buf[b], np * sizeof(float), cudaMemcpyDeviceToHost, ctx->s_copy));
-        FAMSA_CUDA(cudaEventRecord(ctx->ev_copied[b], ctx->s_copy));
+        HostChunkTimers* tm = nullptr;
+        if (g->profile) {
+            g->timers.emplace_back();
+            tm = &g->timers.back();
+            for (cudaEvent_t& ev : tm->ev) HOST_CUDA(cudaEventCreate(&ev));
+            tm->bytes = (double)np * ((lcs_host ? 2 : 0) + (sim_host ? 4 : 0));
+        }
+        if (n >= 2) HOST_CUDA(cudaStreamWaitEvent(g->s_compute, g->ev_copied[b], 0));
+        if (tm) HOST_CUDA(cudaEventRecord(tm->ev[0], g->s_compute));
+        rc = sweep_rows(ctx, r, e, lcs_host ? g->lcs[b] : nullptr, sim_host ? g->sim[b] : nullptr, nullptr, g->s_compute);
+        if (rc != FAMSA_OK) return fail(rc);
+        if (tm) HOST_CUDA(cudaEventRecord(tm->ev[1], g->s_compute));
+        HOST_CUDA(cudaEventRecord(g->ev_done[b], g->s_compute));
+        HOST_CUDA(cudaStreamWaitEvent(g->s_copy, g->ev_done[b], 0));
+        if (tm) HOST_CUDA(cudaEventRecord(tm->ev[2], g->s_copy));
+        if (lcs_host) HOST_CUDA(cudaMemcpyAsync(lcs_host + done_pairs, g->lcs[b], np * sizeof(uint16_t), cudaMemcpyDeviceToHost, g->s_copy));
+        if (sim_host) HOST_CUDA(cudaMemcpyAsync(sim_host + done_pairs, g->sim[b], np * sizeof(float), cudaMemcpyDeviceToHost, g->s_copy));
+        if (tm) HOST_CUDA(cudaEventRecord(tm->ev[3], g->s_copy));
+        HOST_CUDA(cudaEventRecord(g->ev_copied[b], g->s_copy));
         done_pairs += np; r = e; ++n;
     }
     if (wait) {
-        FAMSA_CUDA(cudaStreamSynchronize(ctx->s_copy));
-        FAMSA_CUDA(cudaStreamSynchronize(ctx->s_compute));
+        HOST_CUDA(cudaStreamSynchronize(g->s_copy));
+        HOST_CUDA(cudaStreamSynchronize(g->s_compute));
     }
+#undef HOST_CUDA
     return FAMSA_OK;
 }
 
@@ -486,7 +631,36 @@ extern "C" int famsa_lcs_rows_host_async(famsa_ctx* ctx, int64_t i0, int64_t i1,
 extern "C" int famsa_sync(famsa_ctx* ctx) {
     if (!ctx) { set_error("famsa_sync: ctx is NULL"); return FAMSA_EINVAL; }
     FAMSA_CUDA(cudaSetDevice(ctx->device));
-    if (ctx->s_copy) FAMSA_CUDA(cudaStreamSynchronize(ctx->s_copy));
-    if (ctx->s_compute) FAMSA_CUDA(cudaStreamSynchronize(ctx->s_compute));
+    if (ctx->stg) {
+        FAMSA_CUDA(cudaStreamSynchronize(ctx->stg->s_copy));
+        FAMSA_CUDA(cudaStreamSynchronize(ctx->stg->s_compute));
+    }
+    return FAMSA_OK;
+}
+
+extern "C" int famsa_host_profile(famsa_ctx* ctx, int enable) {
+    if (!ctx) { set_error("famsa_host_profile: ctx is NULL"); return FAMSA_EINVAL; }
+    ctx->host_profile = enable != 0;
+    if (ctx->stg) ctx->stg->profile = ctx->host_profile;
+    return FAMSA_OK;
+}
+
+extern "C" int famsa_host_profile_read(famsa_ctx* ctx, double* out) {
+    if (!ctx || !out) { set_error("famsa_host_profile_read: null argument"); return FAMSA_EINVAL; }
+    for (int q = 0; q < 5; ++q) out[q] = 0.0;
+    if (!ctx->stg || ctx->stg->timers.empty()) return FAMSA_OK;
+    int rc = famsa_sync(ctx);
+    if (rc != FAMSA_OK) return rc;
+    Staging* g = ctx->stg;
+    float ms = 0.0f;
+    for (HostChunkTimers& t : g->timers) {
+        FAMSA_CUDA(cudaEventElapsedTime(&ms, t.ev[0], t.ev[1])); out[0] += ms;
+        FAMSA_CUDA(cudaEventElapsedTime(&ms, t.ev[2], t.ev[3])); out[1] += ms;
+        out[2] += t.bytes;
+    }
+    FAMSA_CUDA(cudaEventElapsedTime(&ms, g->timers.front().ev[0], g->timers.back().ev[3]));
+    out[3] = ms; out[4] = (double)g->timers.size();
+    for (HostChunkTimers& t : g->timers) for (cudaEvent_t e : t.ev) cudaEventDestroy(e);
+    g->timers.clear();
     return FAMSA_OK;
 }

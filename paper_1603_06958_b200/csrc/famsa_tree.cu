@@ -13,6 +13,7 @@
 #include <cub/device/device_radix_sort.cuh>
 
 #include <algorithm>
+#include <cmath>
 #include <new>
 
 #include "famsa_internal.h"
@@ -199,8 +200,8 @@ __global__ void tree_best_kernel(TreeArgs a) {
     } else {
         return;
     }
-    if (w < 0.0f) return;                                   // NO_EDGE
-    const uint32_t key = __float_as_uint(w) + 1u;          // similarities >= 0: bit order == value order
+    if (__float_as_uint(w) & 0x80000000u) return;           // NO_EDGE, or any sign-bit-set weight (-0.0 included)
+    const uint32_t key = __float_as_uint(w) + 1u;          // similarities >= +0: bit order == value order
     const uint32_t cx = a.comp[x];
     if (PASS == 0) {
         atomicMax(&a.best_w[cx], key);
@@ -235,7 +236,11 @@ __global__ void tree_relabel_kernel(TreeArgs a) {
     const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x;
     if (x >= a.n) return;
     uint32_t r = a.comp[x];
-    while (a.parent[r] != r) r = a.parent[r];
+    for (uint32_t p = a.parent[r]; p != r; p = a.parent[r]) {      // hooks form a forest of depth >= 1: climb with
+        const uint32_t g = a.parent[p];                            // pointer jumping (benign race: every write is an
+        if (g != p) a.parent[r] = g;                               // ancestor of r), so chains halve as they are walked
+        r = p;
+    }
     a.comp_next[x] = r;
     if (r == x) atomicAdd(&a.counters[1], 1u);              // x is a root of the new partition
 }
@@ -369,8 +374,8 @@ extern "C" int famsa_tree_merge_edges(famsa_tree* t, const int64_t* a_host, cons
     FAMSA_CUDA(cudaSetDevice(t->device));
     std::vector<uint32_t> a(m), b(m);
     for (int64_t e = 0; e < m; ++e) {
-        if (a_host[e] < 0 || a_host[e] >= t->k || b_host[e] < 0 || b_host[e] >= t->k || !(sim_host[e] >= 0.0f)) {
-            set_error("famsa_tree_merge_edges: edge " + std::to_string(e) + " has a leaf out of range or a negative/NaN similarity");
+        if (a_host[e] < 0 || a_host[e] >= t->k || b_host[e] < 0 || b_host[e] >= t->k || !(sim_host[e] >= 0.0f) || std::signbit(sim_host[e])) {
+            set_error("famsa_tree_merge_edges: edge " + std::to_string(e) + " has a leaf out of range or a negative (-0.0 included) / NaN similarity");
             return FAMSA_ERANGE;
         }
         a[e] = (uint32_t)a_host[e]; b[e] = (uint32_t)b_host[e];
@@ -410,13 +415,11 @@ extern "C" int famsa_tree_edges(famsa_tree* t, int64_t* a_host, int64_t* b_host,
 
 namespace famsa {
 
-__global__ void tree_sortkeys_kernel(uint32_t m, const uint32_t* ta, const uint32_t* tb, const float* tw,
-                                     unsigned long long* id_key, uint32_t* w_key, uint32_t* idx) {
+__global__ void tree_sortkeys_kernel(uint32_t m, const uint32_t* ta, const uint32_t* tb, unsigned long long* id_key, uint32_t* idx) {
     const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= m) return;
     id_key[e] = ((unsigned long long)ta[e] << 32) | tb[e];
     idx[e] = e;
-    (void)tw; (void)w_key;
 }
 __global__ void tree_wkeys_kernel(uint32_t m, const float* tw, const uint32_t* idx, uint32_t* w_key) {
     const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
@@ -488,7 +491,7 @@ extern "C" int famsa_tree_finish(famsa_tree* t, int64_t* id_a_host, int64_t* id_
     FAMSA_CUDA(dalloc((void**)&oa, 8ull * m)); FAMSA_CUDA(dalloc((void**)&ob, 8ull * m)); FAMSA_CUDA(dalloc((void**)&osz, 8ull * m));
     FAMSA_CUDA(dalloc((void**)&ow, 4ull * m));
     const unsigned g = (m + 255) / 256;
-    tree_sortkeys_kernel<<<g, 256>>>(m, t->ta[cur], t->tb[cur], t->tw[cur], idk, wk, idx);
+    tree_sortkeys_kernel<<<g, 256>>>(m, t->ta[cur], t->tb[cur], idk, idx);
     size_t b1 = 0, b2 = 0;                                  // two stable passes: by edge id, then by similarity
     FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, b1, idk, idk2, idx, idx2, (int)m));
     FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, b2, wk, wk2, idx2, order, (int)m));
@@ -549,13 +552,13 @@ extern "C" int famsa_guide_forest(famsa_ctx* ctx, int64_t block_rows, int64_t pa
     GT_CUDA(cudaEventCreateWithFlags(&ev[0], cudaEventDisableTiming));
     GT_CUDA(cudaEventCreateWithFlags(&ev[1], cudaEventDisableTiming));
     rows_of(0, i0, i1);
-    if (famsa_rows_pairs(i0, i1) > 0) GT_TRY(famsa::sweep_rows(ctx, i0, i1, nullptr, buf[0], sa));
+    if (famsa_rows_pairs(i0, i1) > 0) GT_TRY(famsa::sweep_rows(ctx, i0, i1, nullptr, buf[0], nullptr, sa));
     GT_CUDA(cudaEventRecord(ev[0], sa));
     for (int64_t n = 0; n < nb; ++n) {
         if (n + 1 < nb) {                                  // sweep the next block while this one is merged
             int64_t n0, n1;
             rows_of(n + 1, n0, n1);
-            GT_TRY(famsa::sweep_rows(ctx, n0, n1, nullptr, buf[(n + 1) & 1], sa));
+            GT_TRY(famsa::sweep_rows(ctx, n0, n1, nullptr, buf[(n + 1) & 1], nullptr, sa));
             GT_CUDA(cudaEventRecord(ev[(n + 1) & 1], sa));
         }
         rows_of(n, i0, i1);

@@ -15,9 +15,11 @@ LIB_PATH = os.path.join(_HERE, "libfamsa_lcs.so")
 FAMSA_OK, FAMSA_EINVAL, FAMSA_ESYMBOL, FAMSA_ELENGTH, FAMSA_ERANGE, FAMSA_ENOMEM, FAMSA_ECUDA = 0, -1, -2, -3, -4, -5, -6
 FAMSA_MAX_LEN = 65535
 
-EXPORTS = ["famsa_pack", "famsa_lcs_rows", "famsa_lcs_rows_host", "famsa_lcs_rows_host_async", "famsa_sync", "famsa_rows_pairs", "famsa_rows_cells",
+EXPORTS = ["famsa_pack", "famsa_lcs_rows", "famsa_lcs_rows_host", "famsa_lcs_rows_host_async", "famsa_sync",
+           "famsa_lcs_rows_checksum", "famsa_host_profile", "famsa_host_profile_read", "famsa_pack_profile", "famsa_trim",
+           "famsa_rows_pairs", "famsa_rows_cells",
            "famsa_k", "famsa_perm", "famsa_lengths", "famsa_codes", "famsa_match", "famsa_launch_count",
-           "famsa_alu_peak", "famsa_set_tuning", "famsa_free", "famsa_strerror", "famsa_last_error",
+           "famsa_alu_peak", "famsa_mix_peak", "famsa_ctx_set_tuning", "famsa_free", "famsa_strerror", "famsa_last_error",
            "famsa_tree_create", "famsa_tree_update", "famsa_tree_merge_edges", "famsa_tree_edge_count",
            "famsa_tree_edges", "famsa_tree_finish", "famsa_tree_free",
            "famsa_guide_tree", "famsa_guide_forest"]
@@ -69,8 +71,20 @@ def lib():
         L.famsa_launch_count.argtypes = [vp]
         L.famsa_alu_peak.restype = i32
         L.famsa_alu_peak.argtypes = [i32] + [ctypes.POINTER(ctypes.c_double)] * 3
-        L.famsa_set_tuning.restype = i32
-        L.famsa_set_tuning.argtypes = [i32]
+        L.famsa_mix_peak.restype = i32
+        L.famsa_mix_peak.argtypes = [i32] + [ctypes.POINTER(ctypes.c_double)] * 2
+        L.famsa_ctx_set_tuning.restype = i32
+        L.famsa_ctx_set_tuning.argtypes = [vp, i32, i32, i32]
+        L.famsa_lcs_rows_checksum.restype = i32
+        L.famsa_lcs_rows_checksum.argtypes = [vp, i64, i64, vp, vp, vp, vp]
+        L.famsa_host_profile.restype = i32
+        L.famsa_host_profile.argtypes = [vp, i32]
+        L.famsa_host_profile_read.restype = i32
+        L.famsa_host_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+        L.famsa_pack_profile.restype = i32
+        L.famsa_pack_profile.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+        L.famsa_trim.restype = i32
+        L.famsa_trim.argtypes = []
         L.famsa_free.restype = None
         L.famsa_free.argtypes = [vp]
         L.famsa_tree_create.restype = i32
@@ -156,20 +170,35 @@ def famsa_rows_pairs(i0, i1):
     return int(lib().famsa_rows_pairs(int(i0), int(i1)))
 
 
-def famsa_lcs_rows(ctx, i0, i1, lcs_out, sim_out, cuda_stream=None):
-    """lcs_out: torch.uint16/int16 CUDA tensor or None; sim_out: torch.float32 CUDA tensor or None
-    (each with >= famsa_rows_pairs(i0, i1) elements).  Work is enqueued on cuda_stream (an int
-    cudaStream_t, a torch.cuda.Stream, or None = torch's current stream)."""
+def _stream(cuda_stream):
     if cuda_stream is None:
         import torch
-        cuda_stream = torch.cuda.current_stream().cuda_stream
-    elif hasattr(cuda_stream, "cuda_stream"):
-        cuda_stream = cuda_stream.cuda_stream
+        return torch.cuda.current_stream().cuda_stream
+    return cuda_stream.cuda_stream if hasattr(cuda_stream, "cuda_stream") else cuda_stream
+
+
+def _check_device_outputs(i0, i1, lcs_out, sim_out):
     n = famsa_rows_pairs(i0, i1)
     for t, size in ((lcs_out, 2), (sim_out, 4)):
         if t is not None:
             assert t.is_cuda and t.is_contiguous() and t.element_size() == size and t.numel() >= n
-    _check(lib().famsa_lcs_rows(ctx.handle, int(i0), int(i1), _ptr(lcs_out), _ptr(sim_out), cuda_stream))
+
+
+def famsa_lcs_rows(ctx, i0, i1, lcs_out, sim_out, cuda_stream=None):
+    """lcs_out: torch.uint16/int16 CUDA tensor or None; sim_out: torch.float32 CUDA tensor or None
+    (each with >= famsa_rows_pairs(i0, i1) elements).  Work is enqueued on cuda_stream (an int
+    cudaStream_t, a torch.cuda.Stream, or None = torch's current stream)."""
+    _check_device_outputs(i0, i1, lcs_out, sim_out)
+    _check(lib().famsa_lcs_rows(ctx.handle, int(i0), int(i1), _ptr(lcs_out), _ptr(sim_out), _stream(cuda_stream)))
+
+
+def famsa_lcs_rows_checksum(ctx, i0, i1, lcs_out, sim_out, checksum, cuda_stream=None):
+    """As famsa_lcs_rows; `checksum` is a CUDA int64/uint64 tensor of >= 2 elements that the call ADDS to:
+    [0] += sum of LCS, [1] += sum of the similarities' fp32 bit patterns."""
+    _check_device_outputs(i0, i1, lcs_out, sim_out)
+    assert checksum.is_cuda and checksum.is_contiguous() and checksum.element_size() == 8 and checksum.numel() >= 2
+    _check(lib().famsa_lcs_rows_checksum(ctx.handle, int(i0), int(i1), _ptr(lcs_out), _ptr(sim_out), _ptr(checksum),
+                                         _stream(cuda_stream)))
 
 
 def famsa_lcs_rows_host(ctx, i0, i1, lcs_host, sim_host):
@@ -189,8 +218,13 @@ def famsa_lcs_rows_host_async(ctx, i0, i1, lcs_host, sim_host):
     results are in the buffers after famsa_sync(ctx)."""
     n = famsa_rows_pairs(i0, i1)
     for t, size in ((lcs_host, 2), (sim_host, 4)):
-        if t is not None and not isinstance(t, np.ndarray):
+        if t is None:
+            continue
+        if isinstance(t, np.ndarray):                     # a numpy VIEW of pinned memory: size-checked like the sync call;
+            assert t.flags.c_contiguous and t.itemsize == size and t.size >= n    # pageable memory makes the copies synchronous
+        else:
             assert (not t.is_cuda) and t.is_contiguous() and t.element_size() == size and t.numel() >= n
+            assert t.is_pinned(), "famsa_lcs_rows_host_async needs pinned host tensors (pageable memory makes the copies synchronous)"
     _check(lib().famsa_lcs_rows_host_async(ctx.handle, int(i0), int(i1), _ptr(lcs_host), _ptr(sim_host)))
 
 
@@ -245,8 +279,36 @@ def famsa_alu_peak(device=0):
     return {"instr_per_s": a.value, "instr_per_clk_sm": b.value, "sm_mhz": c.value}
 
 
-def famsa_set_tuning(rows_per_cta):
-    _check(lib().famsa_set_tuning(int(rows_per_cta)))
+def famsa_mix_peak(device=0):
+    """Returns dict(alu_instr_per_clk_sm, sm_mhz): the ceiling of the sweep's instruction mix (3 ALU + 1 LDS)."""
+    a, b = ctypes.c_double(), ctypes.c_double()
+    _check(lib().famsa_mix_peak(int(device), ctypes.byref(a), ctypes.byref(b)))
+    return {"alu_instr_per_clk_sm": a.value, "sm_mhz": b.value}
+
+
+def famsa_ctx_set_tuning(ctx, rows_per_cta=0, small_job_mode=-1, l2_group_mb=0):
+    """Per-ctx tuning knobs (0 / -1 = default); results never depend on them."""
+    _check(lib().famsa_ctx_set_tuning(ctx.handle, int(rows_per_cta), int(small_job_mode), int(l2_group_mb)))
+
+
+def famsa_host_profile(ctx, enable=True):
+    _check(lib().famsa_host_profile(ctx.handle, 1 if enable else 0))
+
+
+def famsa_host_profile_read(ctx):
+    out = (ctypes.c_double * 5)()
+    _check(lib().famsa_host_profile_read(ctx.handle, out))
+    return {"sweep_ms": out[0], "d2h_ms": out[1], "d2h_bytes": out[2], "span_ms": out[3], "chunks": int(out[4])}
+
+
+def famsa_pack_profile(ctx):
+    out = (ctypes.c_double * 4)()
+    _check(lib().famsa_pack_profile(ctx.handle, out))
+    return {"h2d_encode_ms": out[0], "sort_ms": out[1], "plan_ms": out[2], "build_ms": out[3]}
+
+
+def famsa_trim():
+    _check(lib().famsa_trim())
 
 
 # ---- stage II consumer: single-linkage guide tree (include/famsa_lcs.h) ----------------------------

@@ -79,7 +79,10 @@ def test_null_ctx_and_strerror(F):
     for code in range(0, -7, -1):
         assert L.famsa_strerror(code).decode() not in ("", "unknown error")
     assert L.famsa_strerror(-99).decode() == "unknown error"
-    assert L.famsa_set_tuning(0) == F.FAMSA_EINVAL
+    assert L.famsa_ctx_set_tuning(None, 0, -1, 0) == F.FAMSA_EINVAL      # the tuning knobs belong to a ctx
+    assert L.famsa_lcs_rows_checksum(None, 0, 0, None, None, None, None) == F.FAMSA_EINVAL
+    assert L.famsa_host_profile(None, 1) == F.FAMSA_EINVAL and L.famsa_host_profile_read(None, None) == F.FAMSA_EINVAL
+    assert L.famsa_trim() == F.FAMSA_OK                                  # nothing pooled: a no-op
 
 
 def test_product_does_not_import_oracle():

@@ -167,11 +167,11 @@ def test_row_block_independence(F, oracle):
                 l, s = gpu_rows(F, ctx, i0, i1)
                 a, b = F.famsa_rows_pairs(0, i0), F.famsa_rows_pairs(0, i1)
                 assert np.array_equal(l, full_lcs[a:b]) and np.array_equal(s, full_sim[a:b])
-        for ta in (1, 3, 12):
-            F.famsa_set_tuning(ta)
+        for ta, small, l2mb in ((1, -1, 0), (3, 0, 1), (12, 0, 0), (8, 0, 4096), (0, 1, 0), (0, 1, 1)):
+            F.famsa_ctx_set_tuning(ctx, ta, small, l2mb)        # tile shapes, one-warp CTAs, L2 column groups
             l, s = gpu_rows(F, ctx, 0, k)
             assert np.array_equal(l, full_lcs) and np.array_equal(s, full_sim)
-        F.famsa_set_tuning(8)
+        F.famsa_ctx_set_tuning(ctx)                             # back to the shipped defaults (the knobs are per ctx)
         l, _ = gpu_rows(F, ctx, 100, 300, want_sim=False)       # LCS only (configs[3])
         _, s = gpu_rows(F, ctx, 100, 300, want_lcs=False)       # similarity only
         a, b = F.famsa_rows_pairs(0, 100), F.famsa_rows_pairs(0, 300)

@@ -195,19 +195,23 @@ def test_sort_perm_and_rows_layout(oracle):
     assert lcs[4 * 3 // 2 + 1] == oracle.lcs_len(seq(4), seq(1))      # entry (4,1) at i(i-1)/2+j
 
 
-def test_bitparallel_cpu_baseline_matches_dp(oracle):
-    """oracle/bitpar_cpu.c is bench.py's context baseline (the paper's own 64-bit CPU design), not an
-    oracle: it must agree with the plain-DP oracle, including 64-bit word boundaries."""
+@pytest.mark.parametrize("isa", [0, 2, 4, 8, -1])
+def test_bitparallel_cpu_baseline_matches_dp(oracle, isa):
+    """oracle/bitpar_cpu.c is bench.py's context baseline (the paper's own 64-bit multi-pair CPU design,
+    PAPER.md:54-56), not an oracle: every lane count (a = 1, 2, 4, 8; the wide ones through the generic code
+    path when the host lacks AVX2 / AVX-512, and natively with isa = -1) must agree with the plain-DP oracle,
+    including 64-bit word boundaries, ragged column lengths inside one vector and partial last vectors."""
     rng = np.random.default_rng(43)
     lens = [1, 2, 63, 64, 65, 127, 128, 129, 300, 1000, 1025] + [int(x) for x in rng.integers(1, 400, 40)]
     seqs = [rng.integers(0, int(rng.choice([2, 4, 25])), n).astype(np.uint8) for n in lens]
     offsets = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
     flat = np.concatenate(seqs)
     k = len(lens)
-    pi, pj = [a.ravel() for a in np.meshgrid(np.arange(k), np.arange(k))]
-    fast = oracle.bitpar_pairs(flat, offsets, pi, pj, n_threads=3)
+    pi, pj = [a.ravel() for a in np.meshgrid(np.arange(k), np.arange(k))]       # 51 columns per row: 51 mod 2, 4, 8 != 0
+    fast = oracle.bitpar_pairs(flat, offsets, pi, pj, isa=isa, n_threads=3)
     slow, _ = oracle.pairs(flat, offsets, pi, pj, want_sim=False, n_threads=3)
     assert np.array_equal(fast, slow)
+    assert oracle.bitpar_best_isa() in oracle.BITPAR_ISA_NAMES
 
 
 def test_oracle_digests_are_stable(oracle):

@@ -112,3 +112,28 @@ def test_invariants():
         if ra != rb:
             parent[ra] = rb; w.append(s)
     assert np.array_equal(so.merge_heights(m), np.array(w))
+
+
+def test_dendrogram_pair_heights_vs_replaying_the_merges():
+    """oracle.slink_oracle.dendrogram_pair_heights (binary-lifting LCA, used by the full-size guide-tree check)
+    against the plain definition: replay the merges in order and note when the two leaves first meet."""
+    from oracle import slink_oracle as so
+    rng = np.random.default_rng(5)
+    for k in (2, 3, 9, 40, 130):
+        n = k * (k - 1) // 2
+        tri = rng.integers(1, 9, n) / 8.0 if k % 2 else rng.random(n)
+        merges = so.single_linkage(so.full_matrix(k, tri))
+        ia = np.array([m[0] for m in merges]); ib = np.array([m[1] for m in merges]); w = np.array([m[2] for m in merges])
+        qi, qj = np.tril_indices(k, -1)
+        got = so.dendrogram_pair_heights(k, ia, ib, w, qi, qj)
+        cluster = {v: {v} for v in range(k)}
+        want = np.full((k, k), np.nan)
+        for t, (a, b, s, _) in enumerate(merges):
+            for x in cluster[a]:
+                for y in cluster[b]:
+                    want[x, y] = want[y, x] = s
+            cluster[k + t] = cluster.pop(a) | cluster.pop(b)
+        assert np.array_equal(got, want[qi, qj])
+        # and the single-linkage property itself: every pair's similarity is at most its merge height
+        S = so.full_matrix(k, tri)
+        assert np.all(S[qi, qj] <= got)
