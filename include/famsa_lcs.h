@@ -80,9 +80,10 @@ int famsa_lcs_rows(famsa_ctx* ctx, int64_t i0, int64_t i1,
                    uint16_t* lcs_out, float* sim_out, void* cuda_stream);
 
 /*
- * famsa_lcs_rows_host -- the same call for HOST output buffers (the end-to-end path):
- * sweeps rows [i0, i1) in row blocks on the device and copies each block back, device
- * compute overlapped with the device->host copy of the previous block.  Synchronous.
+ * famsa_lcs_rows_host -- the same call for HOST output buffers (the end-to-end path).  Synchronous.
+ * Pinned buffers are written by the sweep kernels directly (see famsa_host_mode); for pageable ones the
+ * rows are swept in chunks on the device and each chunk is copied back, device compute overlapped with
+ * the device->host copy of the previous chunk.
  *   lcs_host, sim_host  HOST  as above (either may be NULL, not both); pageable or pinned.
  */
 int famsa_lcs_rows_host(famsa_ctx* ctx, int64_t i0, int64_t i1,
@@ -100,6 +101,17 @@ int famsa_lcs_rows_host_async(famsa_ctx* ctx, int64_t i0, int64_t i1,
 
 /* Wait for everything the host path of this ctx has enqueued. */
 int famsa_sync(famsa_ctx* ctx);
+
+/*
+ * famsa_host_mode -- how famsa_lcs_rows_host* moves the rows to the host (results never depend on it):
+ *   -1  auto (default): if every non-NULL output buffer is PINNED (page-locked and mapped: cudaHostAlloc /
+ *       cudaHostRegister / torch pin_memory), the sweep kernels store each row straight into the caller's
+ *       buffer through its device alias -- the row store of step a7 is then itself the device->host transfer
+ *       (coalesced streaming stores become posted PCIe writes), with no staging buffer, copy engine or chunk
+ *       boundary; pageable buffers take the staged path (device row chunks + cudaMemcpyAsync).
+ *    0  always staged.      1  direct, FAMSA_EINVAL if a buffer is not pinned.
+ */
+int famsa_host_mode(famsa_ctx* ctx, int mode);
 
 /*
  * famsa_lcs_rows_checksum -- famsa_lcs_rows plus a 64-bit checksum of what the call stored (SURVEY.md 8(d):

@@ -89,6 +89,11 @@ struct famsa_ctx {
     famsa::Staging* stg = nullptr;
     int64_t   host_chunks = 0;                  // chunks enqueued by the host path so far
     bool      host_profile = false;
+    // direct host path: PINNED host outputs are written by the sweep kernels themselves (their device alias,
+    // posted PCIe writes), on this stream; no staging, no copy engine, no chunking
+    cudaStream_t s_direct = nullptr;
+    std::atomic<int> host_mode{-1};             // famsa_host_mode: -1 auto (direct if every output is pinned), 0 staged, 1 direct or fail
+    std::deque<famsa::HostChunkTimers> direct_timers;
     // tuning (famsa_ctx_set_tuning): per ctx, so concurrent calls on other ctxs / streams are unaffected
     std::atomic<uint32_t> rows_per_cta{famsa::DEFAULT_ROWS_PER_CTA};
     std::atomic<int>      small_mode{-1};       // -1 auto, 0 never, 1 always: one-warp CTAs, one pair per thread

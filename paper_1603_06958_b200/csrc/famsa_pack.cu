@@ -130,6 +130,8 @@ extern "C" void famsa_free(famsa_ctx* ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     if (ctx->stg) famsa::staging_release(ctx->stg);       // drains the host path's streams, then back to the pool
+    if (ctx->s_direct) { cudaStreamSynchronize(ctx->s_direct); cudaStreamDestroy(ctx->s_direct); }
+    for (famsa::HostChunkTimers& t : ctx->direct_timers) for (cudaEvent_t e : t.ev) if (e) cudaEventDestroy(e);
     cudaFree(ctx->d_stream); cudaFree(ctx->d_tables); cudaFree(ctx->d_len);
     cudaFree(ctx->d_toff); cudaFree(ctx->d_goff);
     delete ctx;

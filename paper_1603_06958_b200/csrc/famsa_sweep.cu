@@ -167,11 +167,19 @@ __device__ __forceinline__ void store_pair(const SweepArgs& a, bool valid, uint3
     const int64_t pos = (int64_t)i * (i - 1) / 2 - a.out_base + j;
     uint32_t sim_bits = 0;
     if (valid) {
+#ifdef EXP_NO_STCS
+        if (a.lcs_out) a.lcs_out[pos] = (unsigned short)lcs;
+#else
         if (a.lcs_out) __stcs(a.lcs_out + pos, (unsigned short)lcs);
+#endif
         if (a.sim_out) {
             const unsigned long long indel = (unsigned long long)la + lb - 2ull * lcs;
             const float sim = __fdiv_rn(__uint2float_rn(lcs), __ull2float_rn(indel * indel));
+#ifdef EXP_NO_STCS
+            a.sim_out[pos] = sim;
+#else
             __stcs(a.sim_out + pos, sim);
+#endif
             sim_bits = __float_as_uint(sim);
         }
     }
@@ -239,12 +247,21 @@ __device__ __forceinline__ void sweep_rows_block(uint32_t (&V)[NR][W], const uin
         word_step_rows<W, NR, TS>(V, q == 0 ? cur.x : (q == 1 ? cur.y : cur.z), tbase);
 }
 
-// Every working warp ends with griddepcontrol.wait: launches after the first one of a call are
-// programmatic dependents (they start while their predecessor drains), and a grid whose CTAs wait for the
-// predecessor's completion cannot itself complete earlier -- so "the last launch of the call is done"
-// implies "every launch of the call is done", which is what an event recorded after the call relies on.
+// Every launch is a PROGRAMMATIC dependent of the kernel before it in the stream (launch_sweep): it may start
+// while its predecessor drains, and every warp executes griddepcontrol.wait BEFORE ITS FIRST STORE (the sweep
+// itself only reads the packed set, which nothing writes after famsa_pack).  The wait returns once the
+// predecessor grid has completed and its memory operations are visible, so (1) stores of consecutive
+// launches -- of one call or of consecutive calls on the stream -- land in stream order even when they hit
+// the same addresses, (2) a grid cannot complete before its predecessor (every launch has at least one
+// storing warp), so "the last launch is done" implies "every launch is done", which is what an event
+// recorded after a call relies on, and (3) a predecessor that is NOT one of these kernels (a consumer of the
+// previous row block, a memcpy) never triggers early, so the launch is then an ordinary stream-ordered one.
 // (Without the launch attribute the instruction is a no-op.)
+#ifdef EXP_NO_PDLWAIT
+__device__ __forceinline__ void pdl_wait() {}
+#else
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+#endif
 
 template <int W, int NR>
 __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
@@ -289,10 +306,10 @@ __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
 #pragma unroll
             for (int w = 0; w < W; ++w) lcs += __popc(~V[p][w]);
             const uint32_t row = i + p;                  // warp-uniform
+            if (p == 0) pdl_wait();                      // stores only after the previous launch is complete
             if (row < r_hi) store_pair(a, j < row, row, j, a.len[row], lb, lcs);
         }
     }
-    pdl_wait();
 }
 
 // ---- blocked path: rows of nblk blocks x W words; one row per CTA; carry bit-vector per thread --
@@ -333,8 +350,8 @@ __global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
         }
     }
     if (active) {
-        store_pair(a, j < i, i, j, a.len[i], j < i ? a.len[j] : 0, lcs);
         pdl_wait();
+        store_pair(a, j < i, i, j, a.len[i], j < i ? a.len[j] : 0, lcs);
     }
 }
 
@@ -343,11 +360,8 @@ __global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
 // ---- host side: buckets -> launches ------------------------------------------------------------
 namespace famsa {
 
-// Launches after the first one of a famsa_lcs_rows call carry the programmatic-stream-serialization
-// attribute: the launches of one call read the same read-only set and write disjoint output ranges,
-// so the next bucket's CTAs may fill the SMs while the previous launch drains its last wave
-// (every sweep kernel executes griddepcontrol.launch_dependents on entry and griddepcontrol.wait at
-// the end of each working warp, see pdl_wait()).
+// Every launch carries the programmatic-stream-serialization attribute (see pdl_wait above): the next
+// bucket's -- or the next call's -- CTAs fill the SMs while the previous launch drains its last wave.
 template <typename K>
 static cudaError_t launch_sweep(K kernel, const SweepArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t st, bool overlap) {
     cudaLaunchConfig_t cfg = {};
@@ -355,7 +369,12 @@ static cudaError_t launch_sweep(K kernel, const SweepArgs& a, unsigned grid, uns
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
+#ifdef EXP_FIRST_SERIAL
     cfg.attrs = attr; cfg.numAttrs = overlap ? 1 : 0;
+#else
+    (void)overlap;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+#endif
     return cudaLaunchKernelEx(&cfg, kernel, a);
 }
 
@@ -557,11 +576,48 @@ extern "C" int famsa_lcs_rows_checksum(famsa_ctx* ctx, int64_t i0, int64_t i1, u
     return sweep_rows(ctx, i0, i1, lcs_out, sim_out, reinterpret_cast<unsigned long long*>(checksum_dev), (cudaStream_t)cuda_stream);
 }
 
+// The device alias of a PINNED (page-locked, mapped) host address, or false for pageable memory.
+static bool pinned_alias(const void* host, void** dev) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, host) != cudaSuccess) { cudaGetLastError(); return false; }
+    if (at.type != cudaMemoryTypeHost || !at.devicePointer) return false;
+    *dev = at.devicePointer;
+    return true;
+}
+
+// Direct host path: the outputs are pinned, so the sweep kernels store each row straight into the caller's
+// buffer through its device alias (coalesced 64 / 128-byte streaming stores become posted PCIe writes; the
+// path produces ~11 GB/s of output against a ~55 GB/s link).  No staging buffers, no copy engine, no chunk
+// boundaries (every chunk boundary of the staged path is a launch that cannot overlap its predecessor's tail).
+static int rows_host_direct(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_dev, float* sim_dev, bool wait) {
+    if (!ctx->s_direct) FAMSA_CUDA(cudaStreamCreateWithFlags(&ctx->s_direct, cudaStreamNonBlocking));
+    HostChunkTimers* tm = nullptr;
+    if (ctx->host_profile) {
+        ctx->direct_timers.emplace_back();
+        tm = &ctx->direct_timers.back();
+        for (int q = 0; q < 2; ++q) FAMSA_CUDA(cudaEventCreate(&tm->ev[q]));
+        tm->bytes = (double)famsa_rows_pairs(i0, i1) * ((lcs_dev ? 2 : 0) + (sim_dev ? 4 : 0));
+        FAMSA_CUDA(cudaEventRecord(tm->ev[0], ctx->s_direct));
+    }
+    int rc = sweep_rows(ctx, i0, i1, lcs_dev, sim_dev, nullptr, ctx->s_direct);
+    if (rc != FAMSA_OK) { cudaStreamSynchronize(ctx->s_direct); return rc; }
+    if (tm) FAMSA_CUDA(cudaEventRecord(tm->ev[1], ctx->s_direct));
+    if (wait) FAMSA_CUDA(cudaStreamSynchronize(ctx->s_direct));
+    return FAMSA_OK;
+}
+
 static int rows_host_impl(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_host, float* sim_host, bool wait) {
     int rc = rows_check(ctx, i0, i1, lcs_host, sim_host, "famsa_lcs_rows_host");
     if (rc != FAMSA_OK) return rc;
     if (famsa_rows_pairs(i0, i1) == 0) return FAMSA_OK;
     FAMSA_CUDA(cudaSetDevice(ctx->device));
+    const int mode = ctx->host_mode.load();
+    if (mode != 0) {
+        void *ld = nullptr, *sd = nullptr;
+        const bool pinned = (!lcs_host || pinned_alias(lcs_host, &ld)) && (!sim_host || pinned_alias(sim_host, &sd));
+        if (pinned) return rows_host_direct(ctx, i0, i1, (uint16_t*)ld, (float*)sd, wait);
+        if (mode == 1) { set_error("famsa_lcs_rows_host: host_mode 1 (direct) needs pinned output buffers"); return FAMSA_EINVAL; }
+    }
     // chunk size: about 1/8 of the call (so the copy of chunk n overlaps the sweep of chunk n+1),
     // between 1 Mi and 128 Mi pairs, and never smaller than the longest row
     const int64_t total_pairs = famsa_rows_pairs(i0, i1);
@@ -635,6 +691,14 @@ extern "C" int famsa_sync(famsa_ctx* ctx) {
         FAMSA_CUDA(cudaStreamSynchronize(ctx->stg->s_copy));
         FAMSA_CUDA(cudaStreamSynchronize(ctx->stg->s_compute));
     }
+    if (ctx->s_direct) FAMSA_CUDA(cudaStreamSynchronize(ctx->s_direct));
+    return FAMSA_OK;
+}
+
+extern "C" int famsa_host_mode(famsa_ctx* ctx, int mode) {
+    if (!ctx) { set_error("famsa_host_mode: ctx is NULL"); return FAMSA_EINVAL; }
+    if (mode < -1 || mode > 1) { set_error("famsa_host_mode: mode must be -1 (auto), 0 (staged) or 1 (direct)"); return FAMSA_EINVAL; }
+    ctx->host_mode.store(mode);
     return FAMSA_OK;
 }
 
@@ -648,11 +712,22 @@ extern "C" int famsa_host_profile(famsa_ctx* ctx, int enable) {
 extern "C" int famsa_host_profile_read(famsa_ctx* ctx, double* out) {
     if (!ctx || !out) { set_error("famsa_host_profile_read: null argument"); return FAMSA_EINVAL; }
     for (int q = 0; q < 5; ++q) out[q] = 0.0;
-    if (!ctx->stg || ctx->stg->timers.empty()) return FAMSA_OK;
     int rc = famsa_sync(ctx);
     if (rc != FAMSA_OK) return rc;
-    Staging* g = ctx->stg;
     float ms = 0.0f;
+    if (!ctx->direct_timers.empty()) {                     // direct path: the stores ARE the transfer, so [1] stays 0
+        for (HostChunkTimers& t : ctx->direct_timers) {
+            FAMSA_CUDA(cudaEventElapsedTime(&ms, t.ev[0], t.ev[1])); out[0] += ms;
+            out[2] += t.bytes;
+        }
+        FAMSA_CUDA(cudaEventElapsedTime(&ms, ctx->direct_timers.front().ev[0], ctx->direct_timers.back().ev[1]));
+        out[3] = ms; out[4] = (double)ctx->direct_timers.size();
+        for (HostChunkTimers& t : ctx->direct_timers) for (cudaEvent_t e : t.ev) if (e) cudaEventDestroy(e);
+        ctx->direct_timers.clear();
+        return FAMSA_OK;
+    }
+    if (!ctx->stg || ctx->stg->timers.empty()) return FAMSA_OK;
+    Staging* g = ctx->stg;
     for (HostChunkTimers& t : g->timers) {
         FAMSA_CUDA(cudaEventElapsedTime(&ms, t.ev[0], t.ev[1])); out[0] += ms;
         FAMSA_CUDA(cudaEventElapsedTime(&ms, t.ev[2], t.ev[3])); out[1] += ms;

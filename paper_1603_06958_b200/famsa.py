@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libfamsa_lcs.so")
 FAMSA_OK, FAMSA_EINVAL, FAMSA_ESYMBOL, FAMSA_ELENGTH, FAMSA_ERANGE, FAMSA_ENOMEM, FAMSA_ECUDA = 0, -1, -2, -3, -4, -5, -6
 FAMSA_MAX_LEN = 65535
 
-EXPORTS = ["famsa_pack", "famsa_lcs_rows", "famsa_lcs_rows_host", "famsa_lcs_rows_host_async", "famsa_sync",
+EXPORTS = ["famsa_pack", "famsa_lcs_rows", "famsa_lcs_rows_host", "famsa_lcs_rows_host_async", "famsa_sync", "famsa_host_mode",
            "famsa_lcs_rows_checksum", "famsa_host_profile", "famsa_host_profile_read", "famsa_pack_profile", "famsa_trim",
            "famsa_rows_pairs", "famsa_rows_cells",
            "famsa_k", "famsa_perm", "famsa_lengths", "famsa_codes", "famsa_match", "famsa_launch_count",
@@ -53,6 +53,8 @@ def lib():
         L.famsa_lcs_rows_host_async.argtypes = [vp, i64, i64, vp, vp]
         L.famsa_sync.restype = i32
         L.famsa_sync.argtypes = [vp]
+        L.famsa_host_mode.restype = i32
+        L.famsa_host_mode.argtypes = [vp, i32]
         L.famsa_rows_pairs.restype = i64
         L.famsa_rows_pairs.argtypes = [i64, i64]
         L.famsa_rows_cells.restype = i32
@@ -230,6 +232,11 @@ def famsa_lcs_rows_host_async(ctx, i0, i1, lcs_host, sim_host):
 
 def famsa_sync(ctx):
     _check(lib().famsa_sync(ctx.handle))
+
+
+def famsa_host_mode(ctx, mode=-1):
+    """-1 auto (pinned outputs are stored by the kernels directly), 0 always staged, 1 direct or fail."""
+    _check(lib().famsa_host_mode(ctx.handle, int(mode)))
 
 
 def famsa_rows_cells(ctx, i0, i1):

@@ -71,6 +71,22 @@ def F():
     return famsa
 
 
+def duplicate_pairs(seqs, offsets, inv_perm):
+    """(i, j < i) in SORTED index space for every pair of byte-identical input sequences (the generator
+    plants three such pairs; they are the entries where indel = 0, R12).  Plain hashing of the
+    input bytes: none of the method's arithmetic."""
+    seen, pi, pj = {}, [], []
+    buf = seqs.tobytes()
+    for t in range(len(offsets) - 1):
+        key = buf[int(offsets[t]):int(offsets[t + 1])]
+        if key in seen:
+            a, b = int(inv_perm[seen[key]]), int(inv_perm[t])
+            pi.append(max(a, b)); pj.append(min(a, b))
+        else:
+            seen[key] = t
+    return np.array(pi, np.int64), np.array(pj, np.int64)
+
+
 def test_config1_full_size_sampled(F, oracle):
     from paper_1603_06958_b200 import synth
     seqs, offsets = synth.family(1)
@@ -101,6 +117,11 @@ def test_config4_one_million_sampled_pairs_of_the_full_sweep(F, oracle, family4)
     with F.famsa_pack(seqs, offsets) as ctx:
         lens = F.famsa_lengths(ctx)
         si, sj = synth.sample_pairs(k, 1_000_000, seed=20260406, lengths_sorted=lens, block_rows=BLOCK_ROWS)
+        inv = np.empty(k, np.int64); inv[perm_ref] = np.arange(k)
+        di, dj = duplicate_pairs(seqs, offsets, inv)                       # the planted duplicates join the sample
+        assert di.size >= 3
+        key = np.unique(np.concatenate([si * k + sj, di * k + dj]))
+        si, sj = key // k, key % k
         assert si.size >= 1_000_000 and np.all(sj < si)
         order = np.argsort(si, kind="stable")
         si, sj = si[order], sj[order]

@@ -323,14 +323,22 @@ def test_host_path_async(F, oracle):
         hl = [torch.empty(mp, dtype=torch.uint16).pin_memory() for _ in range(2)]
         hs = [torch.empty(mp, dtype=torch.float32).pin_memory() for _ in range(2)]
         blocks = [(a, min(a + block, k)) for a in range(0, k, block)]
-        for n in range(0, len(blocks), 2):
-            pair = blocks[n:n + 2]
-            for q, (a, b) in enumerate(pair):
-                F.famsa_lcs_rows_host_async(ctx, a, b, hl[q], hs[q])
-            F.famsa_sync(ctx)
-            for q, (a, b) in enumerate(pair):
-                lo, hi = F.famsa_rows_pairs(0, a), F.famsa_rows_pairs(0, b)
-                assert np.array_equal(hl[q].numpy()[:hi - lo].view(np.uint16), ref_l[lo:hi])
-                assert np.array_equal(hs[q].numpy()[:hi - lo], ref_s[lo:hi])
+        # pinned buffers: mode -1 / 1 = the kernels store into them directly, mode 0 = staged chunks + copies
+        for mode in (-1, 0, 1):
+            F.famsa_host_mode(ctx, mode)
+            for n in range(0, len(blocks), 2):
+                pair = blocks[n:n + 2]
+                for q, (a, b) in enumerate(pair):
+                    hl[q].zero_(); hs[q].zero_()
+                    F.famsa_lcs_rows_host_async(ctx, a, b, hl[q], hs[q] if mode != 1 or n else None)
+                F.famsa_sync(ctx)
+                for q, (a, b) in enumerate(pair):
+                    lo, hi = F.famsa_rows_pairs(0, a), F.famsa_rows_pairs(0, b)
+                    assert np.array_equal(hl[q].numpy()[:hi - lo].view(np.uint16), ref_l[lo:hi])
+                    if mode != 1 or n:
+                        assert np.array_equal(hs[q].numpy()[:hi - lo], ref_s[lo:hi])
+        with pytest.raises(F.FamsaError):                     # direct mode refuses pageable memory
+            F.famsa_lcs_rows_host(ctx, 0, k, ref_l, ref_s)
+        F.famsa_host_mode(ctx, -1)
     lref, sref = oracle.rows(seqs, offsets, 0, k)
     assert_match(ref_l.astype(np.int64), ref_s, lref, sref)
