@@ -195,10 +195,14 @@ int famsa_mix_peak(int device, double* alu_instr_per_clk_sm, double* sm_mhz);
  * built incrementally from the streamed row blocks in O(k) memory ("it can be
  * computed incrementally, i.e., without storing the complete similarity matrix ... first two stages
  * of FAMSA are performed simultaneously").  The paper uses SLINK, whose row update is a serial
- * pointer chase; here the state is the maximum spanning tree of the rows consumed so far (the
- * single-linkage dendrogram is its edges taken by decreasing similarity) and a row block is merged
- * in by data-parallel Boruvka rounds over (old tree edges + the block's dense rows).  Under ties in
- * the similarities the tree is not unique; the sorted merge similarities are.
+ * pointer chase; here the state is the maximum spanning forest of the rows consumed so far (the
+ * single-linkage dendrogram is its edges taken by decreasing similarity).  A row block is merged in
+ * with ONE read of the block and no host round trip: round 0 of Boruvka on the block's own graph
+ * (best entry per row and per column -- the sweep's epilogue delivers these when the block comes from
+ * famsa_guide_forest), one pass that keeps the best edge from every block row into every other
+ * component (at most 1024 components remain after round 0), and a persistent cooperative kernel that
+ * merges the resulting sparse edge set into the forest by Boruvka rounds with grid-wide barriers.
+ * Under ties in the similarities the tree is not unique; the sorted merge similarities are.
  */
 typedef struct famsa_tree famsa_tree;
 
@@ -210,8 +214,11 @@ int famsa_tree_create(int64_t k, int device, famsa_tree** out);
  * once (the state is the maximum spanning forest of the entries seen so far), so a rank of a
  * multi-GPU job can feed only the blocks it swept.
  *   sim_block  DEVICE  famsa_rows_pairs(i0, i1) floats in the famsa_lcs_rows layout, similarities >= 0
- *                      (+inf allowed).  Read on `cuda_stream`; the call returns when the block has
- *                      been merged (it synchronises that stream once per Boruvka round).
+ *                      (+inf allowed; entries with the sign bit set are ignored).
+ * The work is ENQUEUED on `cuda_stream` (NULL = default stream) and not synchronised: sim_block must stay
+ * valid and unchanged until the stream has run; calls for one tree must be stream-ordered with one
+ * another.  famsa_tree_edge_count / _edges / _finish wait for the device.  Errors found on the device
+ * (no convergence, internal overflow) are reported by those calls as FAMSA_EINVAL.
  */
 int famsa_tree_update(famsa_tree* t, int64_t i0, int64_t i1, const float* sim_block, void* cuda_stream);
 
@@ -222,7 +229,8 @@ int famsa_tree_update(famsa_tree* t, int64_t i0, int64_t i1, const float* sim_bl
  */
 int famsa_tree_merge_edges(famsa_tree* t, const int64_t* a_host, const int64_t* b_host, const float* sim_host, int64_t m);
 
-/* Edges in the current forest (k-1 once every row has been consumed or merged in). */
+/* Edges in the current forest (k-1 once every row has been consumed or merged in); waits for the device;
+ * -1 if the device reported an error. */
 int64_t famsa_tree_edge_count(const famsa_tree* t);
 
 /* HOST outputs, famsa_tree_edge_count entries each: the current forest's edges (a > b, leaf indices). */
@@ -240,8 +248,9 @@ void famsa_tree_free(famsa_tree* t);
 
 /*
  * famsa_guide_tree -- stages I and II together, as the paper runs them: sweeps the
- * packed set in row blocks of `block_rows` rows (0 = default 1024) and feeds each block to the tree
- * while the next block is being swept on a second stream; row blocks never leave the device.
+ * packed set in row blocks of `block_rows` rows (0 = default 1024 = the maximum) and feeds each block to
+ * the tree while the next block is being swept on a second stream; row blocks never leave the device and
+ * the host only enqueues (the sweep of block n+2 waits on an event for the merge of block n).
  * Outputs as famsa_tree_finish, in SORTED leaf indices (map through famsa_perm).
  */
 int famsa_guide_tree(famsa_ctx* ctx, int64_t block_rows, int64_t* id_a_host, int64_t* id_b_host,

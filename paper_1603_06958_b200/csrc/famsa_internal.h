@@ -103,9 +103,14 @@ struct famsa_ctx {
 };
 
 namespace famsa {
+// Round-0 candidates of the guide tree (famsa_tree.cu), accumulated by the sweep's epilogue when given:
+// row[i] = max over the row's entries of key(similarity, column), col[j] = max over the call's rows of
+// key(similarity, row); key = (fp32 bits + 1) << 32 | ~other, so a 64-bit atomicMax picks the higher
+// similarity and then the smaller `other`.  The caller zeroes both before the call.
+struct TreeCand { unsigned long long* row; unsigned long long* col; };
 void set_error(const std::string& msg);
 int  cuda_fail(cudaError_t e, const char* what);          // records text, returns FAMSA_ECUDA
-int  sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim, unsigned long long* checksum, cudaStream_t st);
+int  sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim, unsigned long long* checksum, const TreeCand* cand, cudaStream_t st);
 void staging_release(Staging* s);                          // back to the pool (drains its streams first)
 }  // namespace famsa
 

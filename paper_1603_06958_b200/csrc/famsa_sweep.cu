@@ -38,6 +38,8 @@ struct SweepArgs {
     uint32_t        row_tiles;   // row tiles of this launch
     uint32_t        cg_tiles;    // column tiles per column group (L2 blocking of the residue stream, see tile_coords)
     unsigned long long* checksum;   // DEVICE u64[2] or nullptr: += sum of LCS, += sum of similarity bit patterns
+    unsigned long long* cand_row;   // DEVICE or nullptr: round-0 candidates of the guide tree (TreeCand, famsa_internal.h)
+    unsigned long long* cand_col;
 };
 
 // CTA -> (row tile, column tile).  The grid is walked column GROUP by column group: inside a group of
@@ -160,26 +162,20 @@ __device__ __forceinline__ void sweep_block(uint32_t (&V)[W], const uint4* __res
 }
 
 // Epilogue (a6, a7) for one row of a warp: indel = |A| + |B| - 2 LCS, similarity = LCS / indel^2
-// (PAPER.md:42), stored with the streaming hint (st.global.cs: written once, never re-read by the sweep, so
-// the lines should not displace the residue stream in L2).  Called by ALL lanes of the warp (`valid` says
-// which lanes own an entry) so that the optional checksum can use warp reductions.
-__device__ __forceinline__ void store_pair(const SweepArgs& a, bool valid, uint32_t i, uint32_t j, uint32_t la, uint32_t lb, uint32_t lcs) {
+// (PAPER.md:42).  Plain stores: with the column-group rasterisation the residue-stream slice in use stays in L2
+// whatever the output does (measured r02: st.global.cs was 0.3 % slower and saved 0.3 GB of 35 GB DRAM traffic
+// per step).  Called by ALL lanes of the warp (`valid` says which lanes own an entry) so that the optional
+// checksum and the guide tree's candidates can use warp reductions.  Returns the entry as a candidate of
+// column j (0 when candidates are off).
+__device__ __forceinline__ unsigned long long store_pair(const SweepArgs& a, bool valid, uint32_t i, uint32_t j, uint32_t la, uint32_t lb, uint32_t lcs) {
     const int64_t pos = (int64_t)i * (i - 1) / 2 - a.out_base + j;
     uint32_t sim_bits = 0;
     if (valid) {
-#ifdef EXP_NO_STCS
         if (a.lcs_out) a.lcs_out[pos] = (unsigned short)lcs;
-#else
-        if (a.lcs_out) __stcs(a.lcs_out + pos, (unsigned short)lcs);
-#endif
-        if (a.sim_out) {
+        if (a.sim_out || a.cand_row) {
             const unsigned long long indel = (unsigned long long)la + lb - 2ull * lcs;
             const float sim = __fdiv_rn(__uint2float_rn(lcs), __ull2float_rn(indel * indel));
-#ifdef EXP_NO_STCS
-            a.sim_out[pos] = sim;
-#else
-            __stcs(a.sim_out + pos, sim);
-#endif
+            if (a.sim_out) a.sim_out[pos] = sim;
             sim_bits = __float_as_uint(sim);
         }
     }
@@ -189,9 +185,25 @@ __device__ __forceinline__ void store_pair(const SweepArgs& a, bool valid, uint3
         const uint32_t s_hi = __reduce_add_sync(0xffffffffu, sim_bits >> 16);
         if ((threadIdx.x & 31) == 0) {
             if (sl) atomicAdd(a.checksum, (unsigned long long)sl);
-            if (s_lo | s_hi) atomicAdd(a.checksum + 1, ((unsigned long long)s_hi << 16) + s_lo);
+            if (a.sim_out && (s_lo | s_hi)) atomicAdd(a.checksum + 1, ((unsigned long long)s_hi << 16) + s_lo);
         }
     }
+    if (a.cand_row) {                                       // kernel-uniform: the guide tree's round-0 candidates
+        const uint32_t hi = valid ? sim_bits + 1u : 0u;     // similarities are >= +0: bit order == value order
+        const uint32_t hmax = __reduce_max_sync(0xffffffffu, hi);
+        const uint32_t lmax = __reduce_max_sync(0xffffffffu, hi == hmax ? ~j : 0u);    // ties: the smallest column
+        if ((threadIdx.x & 31) == 0 && hmax) {
+            const unsigned long long key = ((unsigned long long)hmax << 32) | lmax;
+            if (key > a.cand_row[i]) atomicMax(a.cand_row + i, key);                   // monotone filter: a stale read only costs an atomic
+        }
+        return valid ? ((unsigned long long)hi << 32) | (uint32_t)~i : 0ull;           // this entry as a candidate of column j
+    }
+    return 0ull;
+}
+
+// Column candidates of one row step of a thread (<= 3 rows): one filtered atomicMax.
+__device__ __forceinline__ void store_col_cand(const SweepArgs& a, uint32_t j, unsigned long long key) {
+    if (key && key > a.cand_col[j]) atomicMax(a.cand_col + j, key);
 }
 
 // ---- register path: every row of the launch fits one block of W words --------------------------
@@ -257,11 +269,7 @@ __device__ __forceinline__ void sweep_rows_block(uint32_t (&V)[NR][W], const uin
 // recorded after a call relies on, and (3) a predecessor that is NOT one of these kernels (a consumer of the
 // previous row block, a memcpy) never triggers early, so the launch is then an ordinary stream-ordered one.
 // (Without the launch attribute the instruction is a no-op.)
-#ifdef EXP_NO_PDLWAIT
-__device__ __forceinline__ void pdl_wait() {}
-#else
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-#endif
 
 template <int W, int NR>
 __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
@@ -300,6 +308,7 @@ __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
 #pragma unroll
             for (int w = 0; w < W; ++w) V[p][w] = 0xFFFFFFFFu;
         sweep_rows_block<W, NR, TS>(V, bp, nwords, smem_base + (i - r_lo) * TS);
+        unsigned long long ckey = 0;
 #pragma unroll
         for (int p = 0; p < NR; ++p) {
             uint32_t lcs = 0;
@@ -307,8 +316,9 @@ __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
             for (int w = 0; w < W; ++w) lcs += __popc(~V[p][w]);
             const uint32_t row = i + p;                  // warp-uniform
             if (p == 0) pdl_wait();                      // stores only after the previous launch is complete
-            if (row < r_hi) store_pair(a, j < row, row, j, a.len[row], lb, lcs);
+            if (row < r_hi) ckey = max(ckey, store_pair(a, j < row, row, j, a.len[row], lb, lcs));
         }
+        if (a.cand_col) store_col_cand(a, j, ckey);
     }
 }
 
@@ -351,7 +361,8 @@ __global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
     }
     if (active) {
         pdl_wait();
-        store_pair(a, j < i, i, j, a.len[i], j < i ? a.len[j] : 0, lcs);
+        const unsigned long long ckey = store_pair(a, j < i, i, j, a.len[i], j < i ? a.len[j] : 0, lcs);
+        if (a.cand_col) store_col_cand(a, j, ckey);
     }
 }
 
@@ -363,24 +374,19 @@ namespace famsa {
 // Every launch carries the programmatic-stream-serialization attribute (see pdl_wait above): the next
 // bucket's -- or the next call's -- CTAs fill the SMs while the previous launch drains its last wave.
 template <typename K>
-static cudaError_t launch_sweep(K kernel, const SweepArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t st, bool overlap) {
+static cudaError_t launch_sweep(K kernel, const SweepArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t st) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
-#ifdef EXP_FIRST_SERIAL
-    cfg.attrs = attr; cfg.numAttrs = overlap ? 1 : 0;
-#else
-    (void)overlap;
     cfg.attrs = attr; cfg.numAttrs = 1;
-#endif
     return cudaLaunchKernelEx(&cfg, kernel, a);
 }
 
-#define SHORT_CASE(W) case W: return small ? launch_sweep(sweep_short_kernel<W, 1>, a, grid, block, smem, st, overlap) \
-                                           : launch_sweep(sweep_short_kernel<W, rows_per_thread(W)>, a, grid, block, smem, st, overlap);
-static cudaError_t dispatch_short(int w, bool small, const SweepArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t st, bool overlap) {
+#define SHORT_CASE(W) case W: return small ? launch_sweep(sweep_short_kernel<W, 1>, a, grid, block, smem, st) \
+                                           : launch_sweep(sweep_short_kernel<W, rows_per_thread(W)>, a, grid, block, smem, st);
+static cudaError_t dispatch_short(int w, bool small, const SweepArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t st) {
     switch (w) {
         SHORT_CASE(1) SHORT_CASE(2) SHORT_CASE(3) SHORT_CASE(4) SHORT_CASE(5) SHORT_CASE(6) SHORT_CASE(7) SHORT_CASE(8)
         SHORT_CASE(9) SHORT_CASE(10) SHORT_CASE(11) SHORT_CASE(12) SHORT_CASE(13) SHORT_CASE(14) SHORT_CASE(15) SHORT_CASE(16)
@@ -389,9 +395,9 @@ static cudaError_t dispatch_short(int w, bool small, const SweepArgs& a, unsigne
         default: return cudaErrorInvalidValue;
     }
 }
-#define LONG_CASE(W) case W: return launch_sweep(sweep_long_kernel<W, CW_SMALL>, a, grid, TB, smem, st, overlap);
-static cudaError_t dispatch_long(int w, bool large, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st, bool overlap) {
-    if (large) return w == 32 ? launch_sweep(sweep_long_kernel<32, CW_LARGE>, a, grid, TB, smem, st, overlap) : cudaErrorInvalidValue;
+#define LONG_CASE(W) case W: return launch_sweep(sweep_long_kernel<W, CW_SMALL>, a, grid, TB, smem, st);
+static cudaError_t dispatch_long(int w, bool large, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st) {
+    if (large) return w == 32 ? launch_sweep(sweep_long_kernel<32, CW_LARGE>, a, grid, TB, smem, st) : cudaErrorInvalidValue;
     switch (w) {
         LONG_CASE(17) LONG_CASE(18) LONG_CASE(19) LONG_CASE(20) LONG_CASE(21) LONG_CASE(22) LONG_CASE(23) LONG_CASE(24)
         LONG_CASE(25) LONG_CASE(26) LONG_CASE(27) LONG_CASE(28) LONG_CASE(29) LONG_CASE(30) LONG_CASE(31) LONG_CASE(32)
@@ -408,7 +414,7 @@ static uint32_t column_group_tiles(const famsa_ctx* ctx, uint32_t r1, uint32_t n
     return (uint32_t)std::min<double>(std::max(t, 1.0), (double)std::max<uint32_t>(n_col_tiles, 1));
 }
 
-int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim, unsigned long long* checksum, cudaStream_t st) {
+int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim, unsigned long long* checksum, const TreeCand* cand, cudaStream_t st) {
     SweepArgs a;
     a.stream = reinterpret_cast<const uint4*>(ctx->d_stream);
     a.goff = ctx->d_goff;
@@ -417,6 +423,7 @@ int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim
     a.len = ctx->d_len;
     a.lcs_out = lcs; a.sim_out = sim;
     a.checksum = checksum;
+    a.cand_row = cand ? cand->row : nullptr; a.cand_col = cand ? cand->col : nullptr;
     a.out_base = i0 * (i0 - 1) / 2;
     const uint32_t rows_per_cta = ctx->rows_per_cta.load();
     const int small_mode = ctx->small_mode.load();
@@ -427,7 +434,6 @@ int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim
     // over 592 sub-partitions) instead of a few fat 128-thread CTAs per SM.
     const bool small = small_mode == 1 || (small_mode < 0 && famsa_rows_pairs(i0, i1) < (int64_t)2048 * ctx->sm_count);
     const unsigned block = small ? 32 : TB;
-    int n_launched = 0;
     for (const Bucket& b : ctx->buckets) {
         int64_t lo = std::max(b.r0, std::max<int64_t>(i0, 1)), hi = std::min(b.r1, i1);   // row 0 is empty
         for (int64_t r = lo; r < hi; r += MAX_ROWS_PER_LAUNCH) {
@@ -442,16 +448,16 @@ int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim
                 while (a.ta > nr && (size_t)(a.ta + nr - 1) * wst * ROW_BYTES + 16 > 48 * 1024) a.ta -= nr;   // default dynamic smem limit
                 a.row_tiles = (a.r1 - a.r0 + a.ta - 1) / a.ta;
                 a.cg_tiles = column_group_tiles(ctx, a.r1, a.n_col_tiles, l2_group_bytes);
-                e = dispatch_short(b.wb, small, a, a.row_tiles * a.n_col_tiles, block, (size_t)(a.ta + nr - 1) * wst * ROW_BYTES + 16, st, n_launched > 0);
+                e = dispatch_short(b.wb, small, a, a.row_tiles * a.n_col_tiles, block, (size_t)(a.ta + nr - 1) * wst * ROW_BYTES + 16, st);
             } else {
                 a.n_col_tiles = (a.r1 - 1 + TB - 1) / TB;
                 a.ta = 1;
                 a.row_tiles = a.r1 - a.r0;
                 a.cg_tiles = column_group_tiles(ctx, a.r1, a.n_col_tiles, l2_group_bytes);
-                e = dispatch_long(b.wb, ctx->large_cw, a, a.row_tiles * a.n_col_tiles, (size_t)wst * ROW_BYTES + 16, st, n_launched > 0);
+                e = dispatch_long(b.wb, ctx->large_cw, a, a.row_tiles * a.n_col_tiles, (size_t)wst * ROW_BYTES + 16, st);
             }
             if (e != cudaSuccess) return cuda_fail(e, "sweep kernel launch");
-            ctx->launches++; ++n_launched;
+            ctx->launches++;
         }
     }
     return FAMSA_OK;
@@ -562,7 +568,7 @@ extern "C" int famsa_lcs_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* 
     if (rc != FAMSA_OK) return rc;
     if (famsa_rows_pairs(i0, i1) == 0) return FAMSA_OK;
     FAMSA_CUDA(cudaSetDevice(ctx->device));
-    return sweep_rows(ctx, i0, i1, lcs_out, sim_out, nullptr, (cudaStream_t)cuda_stream);
+    return sweep_rows(ctx, i0, i1, lcs_out, sim_out, nullptr, nullptr, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int famsa_lcs_rows_checksum(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_out, float* sim_out,
@@ -573,7 +579,7 @@ extern "C" int famsa_lcs_rows_checksum(famsa_ctx* ctx, int64_t i0, int64_t i1, u
     if (famsa_rows_pairs(i0, i1) == 0) return FAMSA_OK;
     FAMSA_CUDA(cudaSetDevice(ctx->device));
     static_assert(sizeof(unsigned long long) == sizeof(uint64_t), "uint64_t");
-    return sweep_rows(ctx, i0, i1, lcs_out, sim_out, reinterpret_cast<unsigned long long*>(checksum_dev), (cudaStream_t)cuda_stream);
+    return sweep_rows(ctx, i0, i1, lcs_out, sim_out, reinterpret_cast<unsigned long long*>(checksum_dev), nullptr, (cudaStream_t)cuda_stream);
 }
 
 // The device alias of a PINNED (page-locked, mapped) host address, or false for pageable memory.
@@ -599,7 +605,7 @@ static int rows_host_direct(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lc
         tm->bytes = (double)famsa_rows_pairs(i0, i1) * ((lcs_dev ? 2 : 0) + (sim_dev ? 4 : 0));
         FAMSA_CUDA(cudaEventRecord(tm->ev[0], ctx->s_direct));
     }
-    int rc = sweep_rows(ctx, i0, i1, lcs_dev, sim_dev, nullptr, ctx->s_direct);
+    int rc = sweep_rows(ctx, i0, i1, lcs_dev, sim_dev, nullptr, nullptr, ctx->s_direct);
     if (rc != FAMSA_OK) { cudaStreamSynchronize(ctx->s_direct); return rc; }
     if (tm) FAMSA_CUDA(cudaEventRecord(tm->ev[1], ctx->s_direct));
     if (wait) FAMSA_CUDA(cudaStreamSynchronize(ctx->s_direct));
@@ -656,7 +662,7 @@ static int rows_host_impl(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs_
         }
         if (n >= 2) HOST_CUDA(cudaStreamWaitEvent(g->s_compute, g->ev_copied[b], 0));
         if (tm) HOST_CUDA(cudaEventRecord(tm->ev[0], g->s_compute));
-        rc = sweep_rows(ctx, r, e, lcs_host ? g->lcs[b] : nullptr, sim_host ? g->sim[b] : nullptr, nullptr, g->s_compute);
+        rc = sweep_rows(ctx, r, e, lcs_host ? g->lcs[b] : nullptr, sim_host ? g->sim[b] : nullptr, nullptr, nullptr, g->s_compute);
         if (rc != FAMSA_OK) return fail(rc);
         if (tm) HOST_CUDA(cudaEventRecord(tm->ev[1], g->s_compute));
         HOST_CUDA(cudaEventRecord(g->ev_done[b], g->s_compute));

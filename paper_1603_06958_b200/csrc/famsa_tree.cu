@@ -4,12 +4,22 @@
 // State: the maximum spanning FOREST T of the similarity entries seen so far (<= k-1 edges).  Single
 // linkage = the spanning tree's edges taken by decreasing similarity, so T is an O(k) summary from which
 // the dendrogram follows, and MSF(E1 u E2) = MSF(MSF(E1) u E2): a row block [i0, i1) -- in any order --
-// is merged in by Boruvka rounds over (T's edges) + (the block's dense entries (v, u < v)); the forests
-// of several ranks are merged the same way from their edge lists (famsa_tree_merge_edges).
-// Every edge has a unique key (similarity descending, then (max, min) endpoint ascending), so each
-// round's picks are edges of the one MSF under that order and only mutual picks form 2-cycles.
-// A round is data-parallel: two streaming passes over the block (best edge per new row, best edge
-// per column), then O(k) per-component reductions with 32/64-bit atomics, hooking and relabelling.
+// is merged in as follows, everything enqueued on the caller's stream, no host round trip:
+//   1. round 0 of Boruvka on the BLOCK's own graph (vertices [0, i1), edges (v, u < v) for the block's rows
+//      v): every vertex picks its best edge -- the best entry of its row and/or of its column.  These
+//      candidates come out of the sweep's own epilogue (64-bit atomicMax keys, famsa_guide_forest) or out of
+//      one pass over the block (famsa_tree_update on a caller's block).  Every component of the pick graph
+//      contains a block row, so there are P <= rows <= 1024 components.
+//   2. ONE pass over the block fills K[row][component] = the best edge from each block row into each OTHER
+//      component (monotone filter: a plain read of the L1/L2-resident table entry, an atomicMax only when the
+//      entry improves, so atomics are ~ entries x ln(columns)).  The picks of 1. plus, per pair of
+//      components, the best entries of K are a sparse edge set S with MSF(T u block) = MSF(T u S): an edge
+//      inside a component, or not the best of its component pair, closes a cycle of heavier edges.
+//   3. a persistent cooperative kernel merges S into T by Boruvka rounds over (T's edges + S) with grid-wide
+//      barriers between the phases, until a round hooks nothing.
+// Every edge has a unique key (similarity descending, then (max, min) endpoint ascending), so each round's
+// picks are edges of the one MSF under that order and only mutual picks form 2-cycles.
+#include <cooperative_groups.h>
 #include <cub/device/device_radix_sort.cuh>
 
 #include <algorithm>
@@ -18,231 +28,315 @@
 
 #include "famsa_internal.h"
 
+namespace cg = cooperative_groups;
+
+namespace famsa {
+
+constexpr int TREE_SUB_ROWS = 1024;    // rows per internal update (bounds the component count P)
+constexpr int KSTRIDE = 1024;          // row stride of the row x component table
+constexpr uint32_t ERR_COMPONENTS = 1, ERR_SPARSE_FULL = 2, ERR_ROUNDS = 4;
+
+// Device-resident scalars of a tree (one struct; the host reads it only when it needs a count).
+struct TreeState {
+    uint32_t m;          // edges of the current forest
+    uint32_t ns;         // edges of the sparse candidate set S of the update in flight
+    uint32_t P;          // components of the block graph after round 0
+    uint32_t err;        // sticky ERR_* flags
+    uint32_t rec;        // edges recorded by the merge in flight
+    uint32_t rounds;     // Boruvka rounds run so far (all merges)
+    uint32_t pad[2];
+};
+
+}  // namespace famsa
+
 struct famsa_tree {
     int      device = 0;
+    int      sm_count = 0;
     int64_t  k = 0;
     int64_t  rows = 0;                 // rows consumed so far (any order)
-    int64_t  max_row_end = 0;          // largest i1 seen: leaves 0..max_row_end-1 are one component
-    int64_t  m = 0;                    // edges of the current forest
-    bool     merged = false;           // sparse edges were merged in: components above max_row_end may exist
-    uint32_t *ta[2] = {nullptr, nullptr}, *tb[2] = {nullptr, nullptr};   // tree edges, a > b (double buffer)
+    bool     merged = false;           // sparse edges were merged in
+    uint32_t *ta[2] = {nullptr, nullptr}, *tb[2] = {nullptr, nullptr};   // forest edges, a > b (double buffer)
     float    *tw[2] = {nullptr, nullptr};
     int      cur = 0;
-    uint32_t *comp[2] = {nullptr, nullptr}, *parent = nullptr;
-    float    *cand_w[2] = {nullptr, nullptr};      // [0] as row owner (new vertices), [1] as column owner
-    uint32_t *cand_o[2] = {nullptr, nullptr};
+    uint32_t *comp[2] = {nullptr, nullptr}, *parent = nullptr;           // merge kernel
     uint32_t *best_w = nullptr;                    // per component: float bits + 1 (0 = none)
     unsigned long long* best_id = nullptr;         // per component: (max << 32) | min of the chosen edge
-    uint32_t *counters = nullptr;                  // [0] edges recorded, [1] roots
-    uint32_t *h_counters = nullptr;                // pinned
-    int64_t  launches = 0, rounds = 0;
+    // block graph (round 0 + row x component table)
+    unsigned long long *cand_row[2] = {nullptr, nullptr}, *cand_col[2] = {nullptr, nullptr};   // two slots: sweep n+1 fills one while update n reads the other
+    unsigned long long *pick = nullptr;            // k
+    uint32_t *bparent = nullptr, *rootidx = nullptr;                     // k each
+    uint16_t *cid16 = nullptr;                     // k: compact component id of the block graph
+    unsigned long long *ktab = nullptr;            // TREE_SUB_ROWS x KSTRIDE
+    uint32_t *wab = nullptr;                       // KSTRIDE x KSTRIDE: best weight key per component pair
+    uint32_t *sa = nullptr, *sb = nullptr; float* sw = nullptr;          // sparse set S
+    size_t   s_cap = 0;
+    famsa::TreeState* st = nullptr;                // device
+    famsa::TreeState* h_st = nullptr;              // pinned
+    int      merge_grid = 0;
+    int64_t  launches = 0;
 };
 
 namespace famsa {
 
-constexpr float NO_EDGE = -1.0f;       // similarities are >= 0
-
-__device__ __forceinline__ bool better(float w, uint32_t o, float bw, uint32_t bo) {
-    return w > bw || (w == bw && o < bo);
+__device__ __forceinline__ unsigned long long cand_key(float w, uint32_t other) {
+    const uint32_t b = __float_as_uint(w);
+    if (b & 0x80000000u) return 0ull;                      // sign bit set (-0.0 included): not an edge
+    return ((unsigned long long)(b + 1u) << 32) | (uint32_t)~other;      // max: higher similarity, then smaller `other`
 }
+__device__ __forceinline__ uint32_t key_other(unsigned long long key) { return ~(uint32_t)key; }
+__device__ __forceinline__ uint32_t key_wbits1(unsigned long long key) { return (uint32_t)(key >> 32); }
 
-// Best edge of each NEW vertex v (a row of the block) to a different component, over columns u < v.
-// A CTA takes ROW_R consecutive rows: one load of comp[u] serves all of them and each thread keeps
-// ROW_R x 4 independent loads in flight.  Measured on a 1.7 GB block: ROW_R = 1 (1024 CTAs) reads 5.7 TB/s,
-// ROW_R = 4 (256 CTAs) only 2.9 TB/s -- the CTA count matters more than sharing comp[u]; ROW_R = 1 is used.
-// HBM-bound: one pass over the block.
-template <int ROW_R>
-__global__ void __launch_bounds__(256) tree_row_kernel(const float* __restrict__ sim, uint32_t i0, uint32_t i1, int64_t out_base,
-                                                       const uint32_t* __restrict__ comp, float* __restrict__ cw, uint32_t* __restrict__ co) {
-    const uint32_t v0 = i0 + blockIdx.x * ROW_R;
-    const float* row[ROW_R]; uint32_t cv[ROW_R], vv[ROW_R];
-    float bw[ROW_R]; uint32_t bo[ROW_R];
-#pragma unroll
-    for (int r = 0; r < ROW_R; ++r) {
-        const uint32_t v = min(v0 + r, i1 - 1);            // rows past the block repeat its last row (not stored)
-        vv[r] = v0 + r < i1 ? v : 0;                       // ... with an empty column range
-        row[r] = sim + ((int64_t)v * (v - 1) / 2 - out_base);
-        cv[r] = comp[v]; bw[r] = NO_EDGE; bo[r] = 0xFFFFFFFFu;
-    }
-    uint32_t vmax = 0;
-#pragma unroll
-    for (int r = 0; r < ROW_R; ++r) vmax = max(vmax, vv[r]);
+// ---- round-0 candidates from a caller's block (famsa_tree_update): one pass, both directions -----------
+// Best entry of each block row v over its columns u < v.  One CTA per row, 4 independent loads in flight per
+// thread (measured r01: 1024 CTAs read a 1.7 GB block at 5.7 TB/s).
+__global__ void __launch_bounds__(256) tree_cand_row_kernel(const float* __restrict__ sim, uint32_t i0, uint32_t i1, int64_t out_base,
+                                                            unsigned long long* __restrict__ cand_row) {
+    const uint32_t v = i0 + blockIdx.x;
+    const float* row = sim + ((int64_t)v * (v - 1) / 2 - out_base);
+    float bw = -1.0f; uint32_t bo = 0xFFFFFFFFu;
 #pragma unroll 4
-    for (uint32_t u = threadIdx.x; u < vmax; u += 256) {
-        const uint32_t c = comp[u];
-        float w[ROW_R];
-#pragma unroll
-        for (int r = 0; r < ROW_R; ++r) w[r] = u < vv[r] ? __ldg(row[r] + u) : NO_EDGE;   // all loads first: ROW_R in flight
-#pragma unroll
-        for (int r = 0; r < ROW_R; ++r)
-            if (c != cv[r] && w[r] > bw[r]) { bw[r] = w[r]; bo[r] = u; }                  // u ascends per thread: first of equals stays
+    for (uint32_t u = threadIdx.x; u < v; u += 256) {
+        const float w = __ldg(row + u);
+        if (w > bw) { bw = w; bo = u; }                    // u ascends per thread: the first of equals stays
     }
-    __shared__ float sw[ROW_R][8];
-    __shared__ uint32_t so[ROW_R][8];
+    unsigned long long key = bo == 0xFFFFFFFFu ? 0ull : cand_key(bw, bo);
 #pragma unroll
-    for (int r = 0; r < ROW_R; ++r) {
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) {
-            const float ow = __shfl_xor_sync(0xffffffffu, bw[r], d);
-            const uint32_t oo = __shfl_xor_sync(0xffffffffu, bo[r], d);
-            if (better(ow, oo, bw[r], bo[r])) { bw[r] = ow; bo[r] = oo; }
-        }
-        if ((threadIdx.x & 31) == 0) { sw[r][threadIdx.x >> 5] = bw[r]; so[r][threadIdx.x >> 5] = bo[r]; }
-    }
+    for (int d = 16; d > 0; d >>= 1) key = max(key, __shfl_xor_sync(0xffffffffu, key, d));
+    __shared__ unsigned long long sk[8];
+    if ((threadIdx.x & 31) == 0) sk[threadIdx.x >> 5] = key;
     __syncthreads();
-    if (threadIdx.x < ROW_R && v0 + threadIdx.x < i1) {
-        const int r = threadIdx.x;
-        float w = sw[r][0]; uint32_t o = so[r][0];
-        for (int q = 1; q < 8; ++q)
-            if (better(sw[r][q], so[r][q], w, o)) { w = sw[r][q]; o = so[r][q]; }
-        cw[v0 + r] = w; co[v0 + r] = o;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int q = 1; q < 8; ++q) key = max(key, sk[q]);
+        cand_row[v] = key;
     }
 }
 
-// Best edge of each vertex u < i1-1 (a column) to a different component, over the block's rows v > u.
-// A CTA covers 64 consecutive columns with 8 row slices (threadIdx.y): consecutive threads read
-// consecutive floats of a row (coalesced), each thread keeps several independent loads in flight, and
-// the 8 slices of a column are combined in shared memory.  HBM-bound: one pass over the block.
+// Best entry of each column u < i1-1 over the block's rows v > u.  A CTA covers 64 consecutive columns with 8
+// row slices (threadIdx.y): consecutive threads read consecutive floats of a row (coalesced).
 constexpr int COL_X = 64, COL_Y = 8;
-__global__ void __launch_bounds__(COL_X * COL_Y) tree_col_kernel(const float* __restrict__ sim, uint32_t i0, uint32_t i1, int64_t out_base,
-                                                                 const uint32_t* __restrict__ comp, float* __restrict__ cw, uint32_t* __restrict__ co) {
-    __shared__ uint32_t scomp[1024];
-    __shared__ float sw[COL_Y][COL_X];
-    __shared__ uint32_t so[COL_Y][COL_X];
-    const uint32_t tid = threadIdx.y * COL_X + threadIdx.x;
+__global__ void __launch_bounds__(COL_X * COL_Y) tree_cand_col_kernel(const float* __restrict__ sim, uint32_t i0, uint32_t i1, int64_t out_base,
+                                                                      unsigned long long* __restrict__ cand_col) {
+    __shared__ unsigned long long sk[COL_Y][COL_X];
     const uint32_t u = blockIdx.x * COL_X + threadIdx.x;
     const bool live = u + 1 < i1;
-    const uint32_t cu = live ? comp[u] : 0;
-    float bw = NO_EDGE; uint32_t bo = 0xFFFFFFFFu;
-    for (uint32_t t0 = i0; t0 < i1; t0 += 1024) {           // the block's rows, 1024 at a time
-        const uint32_t t1 = min(t0 + 1024, i1);
-        __syncthreads();
-        for (uint32_t t = tid; t0 + t < t1; t += COL_X * COL_Y) scomp[t] = comp[t0 + t];
-        __syncthreads();
-        if (live) {
-            // rows v = first + threadIdx.y, + COL_Y, ...  (first = the first row of this pass below column u)
-            const uint32_t first = max(t0, u + 1);
+    float bw = -1.0f; uint32_t bo = 0xFFFFFFFFu;
+    if (live) {
 #pragma unroll 4
-            for (uint32_t v = first + threadIdx.y; v < t1; v += COL_Y) {
-                if (scomp[v - t0] != cu) {
-                    const float w = __ldg(sim + ((int64_t)v * (v - 1) / 2 - out_base + u));
-                    if (w > bw) { bw = w; bo = v; }          // v ascends within a slice: the first of equal weights stays
-                }
-            }
+        for (uint32_t v = max(i0, u + 1) + threadIdx.y; v < i1; v += COL_Y) {
+            const float w = __ldg(sim + ((int64_t)v * (v - 1) / 2 - out_base + u));
+            if (w > bw) { bw = w; bo = v; }                // v ascends within a slice
         }
     }
-    sw[threadIdx.y][threadIdx.x] = bw; so[threadIdx.y][threadIdx.x] = bo;
+    sk[threadIdx.y][threadIdx.x] = bo == 0xFFFFFFFFu ? 0ull : cand_key(bw, bo);
     __syncthreads();
     if (threadIdx.y == 0 && live) {
+        unsigned long long key = sk[0][threadIdx.x];
 #pragma unroll
-        for (int q = 1; q < COL_Y; ++q)
-            if (better(sw[q][threadIdx.x], so[q][threadIdx.x], bw, bo)) { bw = sw[q][threadIdx.x]; bo = so[q][threadIdx.x]; }
-        cw[u] = bw; co[u] = bo;
+        for (int q = 1; q < COL_Y; ++q) key = max(key, sk[q][threadIdx.x]);
+        cand_col[u] = key;
     }
 }
 
-}  // namespace famsa
+struct BlockArgs {
+    uint32_t i0, i1;             // rows of the (sub-)block
+    const unsigned long long *cand_row, *cand_col;
+    unsigned long long* pick;
+    uint32_t *bparent, *rootidx;
+    uint16_t* cid16;
+    unsigned long long* ktab;
+    uint32_t* wab;
+    uint32_t *sa, *sb; float* sw; uint32_t s_cap;
+    TreeState* st;
+};
 
-namespace famsa {
+// Round 0 on the block graph: every vertex x < i1 picks the better of its row and column candidates.
+__global__ void tree_pick_kernel(BlockArgs a) {
+    const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x == 0) { a.st->P = 0; a.st->ns = 0; }
+    if (x >= a.i1) return;
+    const unsigned long long kr = x >= a.i0 ? a.cand_row[x] : 0ull;
+    const unsigned long long kc = x + 1 < a.i1 ? a.cand_col[x] : 0ull;
+    a.pick[x] = max(kr, kc);
+}
 
-struct TreeArgs {
-    uint32_t n;                 // all k leaves
-    uint32_t i0, i1;            // rows of the dense block (i0 == i1: none)
-    uint32_t m;                 // edges of the current forest
-    uint32_t xm;                // extra sparse edges (famsa_tree_merge_edges)
-    const uint32_t *xa, *xb; const float* xw;
-    const uint32_t *ta, *tb; const float* tw;            // current forest
-    uint32_t *na, *nb; float* nw;                        // new tree being recorded
-    const uint32_t* comp; uint32_t* comp_next; uint32_t* parent;
-    const float *cw_row, *cw_col; const uint32_t *co_row, *co_col;
+// Hooking: x -> the other end of its pick; of a mutual pair the smaller index stays a root.  Every pick is an
+// edge of the block graph's MSF (it is the best edge of a vertex) and is recorded once into S.
+__global__ void tree_hook0_kernel(BlockArgs a) {
+    const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= a.i1) return;
+    const unsigned long long key = a.pick[x];
+    if (key == 0) { a.bparent[x] = x; return; }             // no edge at all (a one-row block of row 0)
+    const uint32_t y = key_other(key);
+    const bool mutual = a.pick[y] == ((key & 0xFFFFFFFF00000000ull) | (uint32_t)~x);
+    if (mutual && x < y) { a.bparent[x] = x; return; }
+    a.bparent[x] = y;
+    const uint32_t pos = atomicAdd(&a.st->ns, 1u);
+    if (pos < a.s_cap) { a.sa[pos] = max(x, y); a.sb[pos] = min(x, y); a.sw[pos] = __uint_as_float(key_wbits1(key) - 1u); }
+    else atomicOr(&a.st->err, ERR_SPARSE_FULL);
+}
+
+// Component roots by pointer jumping (benign race: every write is an ancestor); roots get compact ids.
+__global__ void tree_root0_kernel(BlockArgs a) {
+    const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= a.i1) return;
+    uint32_t r = x;
+    for (uint32_t p = a.bparent[r]; p != r; p = a.bparent[r]) {
+        const uint32_t g = a.bparent[p];
+        if (g != p) a.bparent[r] = g;
+        r = p;
+    }
+    a.pick[x] = r;                                           // reuse: the root of x
+    if (r == x) {
+        const uint32_t id = atomicAdd(&a.st->P, 1u);
+        if (id >= (uint32_t)KSTRIDE) atomicOr(&a.st->err, ERR_COMPONENTS);    // cannot happen: every component holds a block row
+        a.rootidx[x] = id;
+    }
+}
+__global__ void tree_cid_kernel(BlockArgs a) {
+    const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= a.i1) return;
+    a.cid16[x] = (uint16_t)min(a.rootidx[(uint32_t)a.pick[x]], (uint32_t)KSTRIDE - 1);
+}
+
+// The one pass over the block: K[row][component b] = best edge from block row v into component b != comp(v).
+// One CTA per row.  The table row (P x 8 B <= 8 KB) stays in L1/L2; an entry is read with a plain load and
+// only an improving key goes to atomicMax (a stale read only costs a redundant atomic).  HBM-bound: one
+// read of the block + 2 B of (L2-resident) component id per entry.
+__global__ void __launch_bounds__(256) tree_rowcomp_kernel(const float* __restrict__ sim, uint32_t i0, uint32_t i1, int64_t out_base, BlockArgs a) {
+    if (a.st->P <= 1) return;                               // the block graph is already connected
+    const uint32_t v = i0 + blockIdx.x;
+    const float* row = sim + ((int64_t)v * (v - 1) / 2 - out_base);
+    const uint16_t ca = a.cid16[v];
+    unsigned long long* krow = a.ktab + (size_t)blockIdx.x * KSTRIDE;
+    const uint16_t* __restrict__ cid = a.cid16;
+    uint32_t u = threadIdx.x;
+    for (; u + 768 < v; u += 1024) {                        // 4 independent loads in flight
+        float w[4]; uint16_t c[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { w[q] = __ldg(row + u + q * 256); c[q] = cid[u + q * 256]; }
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            if (c[q] != ca) {
+                const unsigned long long key = cand_key(w[q], u + q * 256);
+                if (key > krow[c[q]]) atomicMax(&krow[c[q]], key);
+            }
+    }
+    for (; u < v; u += 256) {
+        const float w = __ldg(row + u); const uint16_t c = cid[u];
+        if (c != ca) {
+            const unsigned long long key = cand_key(w, u);
+            if (key > krow[c]) atomicMax(&krow[c], key);
+        }
+    }
+}
+
+// S += the best entries of K per pair of components (ties keep several: harmless).
+template <int PASS>
+__global__ void tree_gather_kernel(BlockArgs a) {
+    const uint32_t P = a.st->P;
+    if (P <= 1) return;
+    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t vi = t / KSTRIDE, b = t % KSTRIDE;
+    if (vi >= a.i1 - a.i0 || b >= P) return;
+    const unsigned long long key = a.ktab[t];
+    if (key == 0) return;
+    const uint32_t v = a.i0 + vi, ca = a.cid16[v];
+    uint32_t* wslot = &a.wab[min(ca, b) * KSTRIDE + max(ca, b)];
+    if (PASS == 0) { atomicMax(wslot, key_wbits1(key)); return; }
+    if (*wslot != key_wbits1(key)) return;
+    const uint32_t u = key_other(key);
+    const uint32_t pos = atomicAdd(&a.st->ns, 1u);
+    if (pos < a.s_cap) { a.sa[pos] = v; a.sb[pos] = u; a.sw[pos] = __uint_as_float(key_wbits1(key) - 1u); }
+    else atomicOr(&a.st->err, ERR_SPARSE_FULL);
+}
+
+// ---- the merge: MSF(T u S) by Boruvka rounds, one persistent cooperative kernel ------------------------
+struct MergeArgs {
+    uint32_t n;                                            // all k leaves
+    const uint32_t *ta, *tb; const float* tw;              // current forest (st->m edges)
+    const uint32_t *sa, *sb; const float* sw;              // sparse set S (st->ns edges)
+    uint32_t *na, *nb; float* nw;                          // the new forest
+    uint32_t *comp0, *comp1, *parent;
     uint32_t* best_w; unsigned long long* best_id;
-    uint32_t* counters;
+    TreeState* st;
 };
 
 __device__ __forceinline__ unsigned long long edge_id(uint32_t x, uint32_t y) {
     return ((unsigned long long)max(x, y) << 32) | min(x, y);
 }
 
-__global__ void tree_reset_kernel(TreeArgs a, int first) {
-    const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x;
-    if (x < a.n) {
-        a.best_w[x] = 0; a.best_id[x] = ~0ull;
-        if (first) const_cast<uint32_t*>(a.comp)[x] = x;
+__global__ void __launch_bounds__(256) tree_merge_kernel(MergeArgs a) {
+    cg::grid_group grid = cg::this_grid();
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    const uint32_t m = a.st->m, ns = a.st->ns, items = m + ns;
+    uint32_t* comp = a.comp0; uint32_t* comp_next = a.comp1;
+    for (uint32_t x = tid; x < a.n; x += nth) comp[x] = x;
+    grid.sync();                                           // (everyone has read st->m / st->ns before rec is reset)
+    if (tid == 0) a.st->rec = 0;
+    uint32_t recorded = 0, round = 0;
+    for (;; ++round) {
+        for (uint32_t x = tid; x < a.n; x += nth) { a.best_w[x] = 0; a.best_id[x] = ~0ull; }
+        grid.sync();
+        // per component: the highest similarity of an outgoing edge ...
+        for (uint32_t e = tid; e < items; e += nth) {
+            const uint32_t x = e < m ? a.ta[e] : a.sa[e - m], y = e < m ? a.tb[e] : a.sb[e - m];
+            const uint32_t wb = __float_as_uint(e < m ? a.tw[e] : a.sw[e - m]);
+            if (x == y || (wb & 0x80000000u)) continue;
+            const uint32_t cx = comp[x], cy = comp[y];
+            if (cx == cy) continue;
+            atomicMax(&a.best_w[cx], wb + 1u); atomicMax(&a.best_w[cy], wb + 1u);
+        }
+        grid.sync();
+        // ... and among the edges that reach it, the smallest edge id: the component's minimum-key outgoing edge
+        for (uint32_t e = tid; e < items; e += nth) {
+            const uint32_t x = e < m ? a.ta[e] : a.sa[e - m], y = e < m ? a.tb[e] : a.sb[e - m];
+            const uint32_t wb = __float_as_uint(e < m ? a.tw[e] : a.sw[e - m]);
+            if (x == y || (wb & 0x80000000u)) continue;
+            const uint32_t cx = comp[x], cy = comp[y];
+            if (cx == cy) continue;
+            const unsigned long long id = edge_id(x, y);
+            if (a.best_w[cx] == wb + 1u) atomicMin(&a.best_id[cx], id);
+            if (a.best_w[cy] == wb + 1u) atomicMin(&a.best_id[cy], id);
+        }
+        grid.sync();
+        // each component root hooks onto the component at the other end of its edge (mutual picks: the smaller
+        // root stays) and records the edge once
+        for (uint32_t c = tid; c < a.n; c += nth) {
+            uint32_t p = c;
+            if (comp[c] == c && a.best_w[c] != 0) {
+                const unsigned long long id = a.best_id[c];
+                const uint32_t hi = (uint32_t)(id >> 32), lo = (uint32_t)id;
+                const uint32_t t = comp[comp[hi] == c ? lo : hi];
+                if (!(a.best_id[t] == id && c < t)) {
+                    p = t;
+                    const uint32_t pos = atomicAdd(&a.st->rec, 1u);
+                    a.na[pos] = hi; a.nb[pos] = lo; a.nw[pos] = __uint_as_float(a.best_w[c] - 1u);
+                }
+            }
+            a.parent[c] = p;
+        }
+        grid.sync();
+        const uint32_t rec = *(volatile uint32_t*)&a.st->rec;
+        const bool done = rec == recorded;                   // a round that hooks nothing: done
+        recorded = rec;
+        if (done || round >= 63) break;
+        for (uint32_t x = tid; x < a.n; x += nth) {
+            uint32_t r = comp[x];
+            for (uint32_t p = a.parent[r]; p != r; p = a.parent[r]) {     // pointer jumping (benign race: every
+                const uint32_t g = a.parent[p];                            // write is an ancestor of r)
+                if (g != p) a.parent[r] = g;
+                r = p;
+            }
+            comp_next[x] = r;
+        }
+        grid.sync();
+        uint32_t* s = comp; comp = comp_next; comp_next = s;
     }
-    if (x == 0) { a.counters[1] = 0; if (first) a.counters[0] = 0; }
-}
-
-// Items: [0, n) row candidates, [n, 2n) column candidates, [2n, 2n+m) forest edges, then xm extra edges.
-// PASS 0: per component, the highest similarity of an outgoing edge.  PASS 1: among the edges that
-// reach it, the smallest edge id.  Together: the component's minimum-key outgoing edge.
-template <int PASS>
-__global__ void tree_best_kernel(TreeArgs a) {
-    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
-    uint32_t x, y; float w;
-    bool both = false;
-    if (t < a.n) {
-        if (t < a.i0 || t >= a.i1) return;
-        x = t; w = a.cw_row[t]; y = a.co_row[t];
-    } else if (t < 2 * a.n) {
-        x = t - a.n;
-        if (a.i1 == a.i0 || x + 1 >= a.i1) return;
-        w = a.cw_col[x]; y = a.co_col[x];
-    } else if (t < 2 * a.n + a.m) {
-        const uint32_t e = t - 2 * a.n;
-        x = a.ta[e]; y = a.tb[e]; w = a.tw[e];
-        if (a.comp[x] == a.comp[y]) return;
-        both = true;
-    } else if (t < 2 * a.n + a.m + a.xm) {
-        const uint32_t e = t - 2 * a.n - a.m;
-        x = a.xa[e]; y = a.xb[e]; w = a.xw[e];
-        if (x == y || a.comp[x] == a.comp[y]) return;
-        both = true;
-    } else {
-        return;
+    if (tid == 0) {
+        a.st->m = recorded; a.st->ns = 0; a.st->rounds += round + 1;
+        if (round >= 63) atomicOr(&a.st->err, ERR_ROUNDS);
     }
-    if (__float_as_uint(w) & 0x80000000u) return;           // NO_EDGE, or any sign-bit-set weight (-0.0 included)
-    const uint32_t key = __float_as_uint(w) + 1u;          // similarities >= +0: bit order == value order
-    const uint32_t cx = a.comp[x];
-    if (PASS == 0) {
-        atomicMax(&a.best_w[cx], key);
-        if (both) atomicMax(&a.best_w[a.comp[y]], key);
-    } else {
-        const unsigned long long id = edge_id(x, y);
-        if (a.best_w[cx] == key) atomicMin(&a.best_id[cx], id);
-        if (both) { const uint32_t cy = a.comp[y]; if (a.best_w[cy] == key) atomicMin(&a.best_id[cy], id); }
-    }
-}
-
-// Each component root hooks onto the component at the other end of its edge (mutual picks: the
-// smaller root stays) and records the edge once.
-__global__ void tree_hook_kernel(TreeArgs a) {
-    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= a.n) return;
-    if (a.comp[c] != c) { a.parent[c] = c; return; }        // not a representative
-    const uint32_t key = a.best_w[c];
-    if (key == 0) { a.parent[c] = c; return; }              // no outgoing edge: the last component
-    const unsigned long long id = a.best_id[c];
-    const uint32_t hi = (uint32_t)(id >> 32), lo = (uint32_t)id;
-    const uint32_t other = a.comp[hi] == c ? lo : hi;
-    const uint32_t t = a.comp[other];
-    const bool mutual = a.best_id[t] == id;
-    if (mutual && c < t) { a.parent[c] = c; return; }       // t hooks onto c and records the edge
-    a.parent[c] = t;
-    const uint32_t pos = atomicAdd(&a.counters[0], 1u);
-    a.na[pos] = hi; a.nb[pos] = lo; a.nw[pos] = __uint_as_float(key - 1u);
-}
-
-__global__ void tree_relabel_kernel(TreeArgs a) {
-    const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x;
-    if (x >= a.n) return;
-    uint32_t r = a.comp[x];
-    for (uint32_t p = a.parent[r]; p != r; p = a.parent[r]) {      // hooks form a forest of depth >= 1: climb with
-        const uint32_t g = a.parent[p];                            // pointer jumping (benign race: every write is an
-        if (g != p) a.parent[r] = g;                               // ancestor of r), so chains halve as they are walked
-        r = p;
-    }
-    a.comp_next[x] = r;
-    if (r == x) atomicAdd(&a.counters[1], 1u);              // x is a root of the new partition
 }
 
 template <typename T>
@@ -250,6 +344,80 @@ static int tree_alloc(T** p, size_t n) {
     cudaError_t e = cudaMalloc((void**)p, std::max<size_t>(n, 1) * sizeof(T));
     if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); set_error("famsa_tree: device allocation failed"); return FAMSA_ENOMEM; }
     if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc");
+    return FAMSA_OK;
+}
+
+static BlockArgs block_args(famsa_tree* t, int64_t i0, int64_t i1, int slot) {
+    BlockArgs a;
+    a.i0 = (uint32_t)i0; a.i1 = (uint32_t)i1;
+    a.cand_row = t->cand_row[slot]; a.cand_col = t->cand_col[slot];
+    a.pick = t->pick; a.bparent = t->bparent; a.rootidx = t->rootidx; a.cid16 = t->cid16;
+    a.ktab = t->ktab; a.wab = t->wab;
+    a.sa = t->sa; a.sb = t->sb; a.sw = t->sw; a.s_cap = (uint32_t)t->s_cap;
+    a.st = t->st;
+    return a;
+}
+
+// MSF(T u S) -> the other forest buffer; flips t->cur.  Enqueue only.
+static int tree_merge(famsa_tree* t, cudaStream_t st) {
+    const int cur = t->cur, nxt = cur ^ 1;
+    MergeArgs a;
+    a.n = (uint32_t)t->k;
+    a.ta = t->ta[cur]; a.tb = t->tb[cur]; a.tw = t->tw[cur];
+    a.sa = t->sa; a.sb = t->sb; a.sw = t->sw;
+    a.na = t->ta[nxt]; a.nb = t->tb[nxt]; a.nw = t->tw[nxt];
+    a.comp0 = t->comp[0]; a.comp1 = t->comp[1]; a.parent = t->parent;
+    a.best_w = t->best_w; a.best_id = t->best_id; a.st = t->st;
+    void* args[] = {&a};
+    FAMSA_CUDA(cudaLaunchCooperativeKernel((const void*)tree_merge_kernel, dim3((unsigned)t->merge_grid), dim3(256), args, 0, st));
+    t->launches++;
+    t->cur = nxt;
+    return FAMSA_OK;
+}
+
+// One (sub-)block of <= TREE_SUB_ROWS rows: candidates are in slot `slot` (fused == true: the sweep's
+// epilogue put them there) or are computed from the block here.  Enqueue only.
+int tree_consume(famsa_tree* t, int64_t i0, int64_t i1, const float* sim, int64_t out_base, int slot, bool fused, cudaStream_t st) {
+    const BlockArgs a = block_args(t, i0, i1, slot);
+    const unsigned gv = (unsigned)((i1 + 255) / 256);
+    if (!fused) {
+        tree_cand_row_kernel<<<(unsigned)(i1 - i0), 256, 0, st>>>(sim, a.i0, a.i1, out_base, t->cand_row[slot]);
+        if (i1 >= 2) tree_cand_col_kernel<<<(unsigned)((i1 - 1 + COL_X - 1) / COL_X), dim3(COL_X, COL_Y), 0, st>>>(sim, a.i0, a.i1, out_base, t->cand_col[slot]);
+        t->launches += 2;
+    }
+    tree_pick_kernel<<<gv, 256, 0, st>>>(a);
+    tree_hook0_kernel<<<gv, 256, 0, st>>>(a);
+    tree_root0_kernel<<<gv, 256, 0, st>>>(a);
+    tree_cid_kernel<<<gv, 256, 0, st>>>(a);
+    FAMSA_CUDA(cudaMemsetAsync(t->ktab, 0, sizeof(unsigned long long) * (size_t)(i1 - i0) * KSTRIDE, st));
+    FAMSA_CUDA(cudaMemsetAsync(t->wab, 0, sizeof(uint32_t) * (size_t)KSTRIDE * KSTRIDE, st));
+    tree_rowcomp_kernel<<<(unsigned)(i1 - i0), 256, 0, st>>>(sim, a.i0, a.i1, out_base, a);
+    const unsigned gk = (unsigned)(((size_t)(i1 - i0) * KSTRIDE + 255) / 256);
+    tree_gather_kernel<0><<<gk, 256, 0, st>>>(a);
+    tree_gather_kernel<1><<<gk, 256, 0, st>>>(a);
+    t->launches += 7;
+    FAMSA_CUDA(cudaGetLastError());
+    return tree_merge(t, st);
+}
+
+// Zero the candidate slot for rows [i0, i1) before the sweep's epilogue accumulates into it.
+int tree_fused_begin(famsa_tree* t, int64_t i0, int64_t i1, int slot, cudaStream_t st) {
+    FAMSA_CUDA(cudaMemsetAsync(t->cand_row[slot] + i0, 0, sizeof(unsigned long long) * (size_t)(i1 - i0), st));
+    FAMSA_CUDA(cudaMemsetAsync(t->cand_col[slot], 0, sizeof(unsigned long long) * (size_t)i1, st));
+    return FAMSA_OK;
+}
+
+// Wait for the tree's work and fetch its device scalars.
+static int tree_read_state(famsa_tree* t) {
+    FAMSA_CUDA(cudaSetDevice(t->device));
+    FAMSA_CUDA(cudaDeviceSynchronize());
+    FAMSA_CUDA(cudaMemcpy(t->h_st, t->st, sizeof(TreeState), cudaMemcpyDeviceToHost));
+    if (t->h_st->err) {
+        set_error(std::string("famsa_tree: the device reported") + ((t->h_st->err & ERR_ROUNDS) ? " no convergence after 64 Boruvka rounds" : "") +
+                  ((t->h_st->err & ERR_SPARSE_FULL) ? " an overflow of the sparse candidate set" : "") +
+                  ((t->h_st->err & ERR_COMPONENTS) ? " more block components than block rows" : ""));
+        return FAMSA_EINVAL;
+    }
     return FAMSA_OK;
 }
 
@@ -262,12 +430,15 @@ using namespace famsa;
 extern "C" void famsa_tree_free(famsa_tree* t) {
     if (!t) return;
     cudaSetDevice(t->device);
+    cudaDeviceSynchronize();
     for (int b = 0; b < 2; ++b) {
         cudaFree(t->ta[b]); cudaFree(t->tb[b]); cudaFree(t->tw[b]); cudaFree(t->comp[b]);
-        cudaFree(t->cand_w[b]); cudaFree(t->cand_o[b]);
+        cudaFree(t->cand_row[b]); cudaFree(t->cand_col[b]);
     }
-    cudaFree(t->parent); cudaFree(t->best_w); cudaFree(t->best_id); cudaFree(t->counters);
-    if (t->h_counters) cudaFreeHost(t->h_counters);
+    cudaFree(t->parent); cudaFree(t->best_w); cudaFree(t->best_id);
+    cudaFree(t->pick); cudaFree(t->bparent); cudaFree(t->rootidx); cudaFree(t->cid16);
+    cudaFree(t->ktab); cudaFree(t->wab); cudaFree(t->sa); cudaFree(t->sb); cudaFree(t->sw); cudaFree(t->st);
+    if (t->h_st) cudaFreeHost(t->h_st);
     delete t;
 }
 
@@ -283,74 +454,32 @@ extern "C" int famsa_tree_create(int64_t k, int device, famsa_tree** out) {
     famsa_tree* t = new (std::nothrow) famsa_tree();
     if (!t) { set_error("famsa_tree_create: host allocation failed"); return FAMSA_ENOMEM; }
     t->device = device; t->k = k;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); famsa_tree_free(t); set_error("famsa_tree_create: cudaGetDeviceProperties"); return FAMSA_ECUDA; }
+    t->sm_count = prop.multiProcessorCount;
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tree_merge_kernel, 256, 0) != cudaSuccess || per_sm < 1 || !prop.cooperativeLaunch) {
+        cudaGetLastError(); famsa_tree_free(t); set_error("famsa_tree_create: the device cannot run the cooperative merge kernel"); return FAMSA_ECUDA;
+    }
+    t->merge_grid = t->sm_count;                           // one 256-thread CTA per SM: co-resident beside the sweep's CTAs
     const size_t n = (size_t)k;
     for (int b = 0; b < 2; ++b) {
         TREE_TRY(tree_alloc(&t->ta[b], n)); TREE_TRY(tree_alloc(&t->tb[b], n)); TREE_TRY(tree_alloc(&t->tw[b], n));
-        TREE_TRY(tree_alloc(&t->comp[b], n)); TREE_TRY(tree_alloc(&t->cand_w[b], n)); TREE_TRY(tree_alloc(&t->cand_o[b], n));
+        TREE_TRY(tree_alloc(&t->comp[b], n)); TREE_TRY(tree_alloc(&t->cand_row[b], n)); TREE_TRY(tree_alloc(&t->cand_col[b], n));
     }
     TREE_TRY(tree_alloc(&t->parent, n)); TREE_TRY(tree_alloc(&t->best_w, n)); TREE_TRY(tree_alloc(&t->best_id, n));
-    TREE_TRY(tree_alloc(&t->counters, 2));
-    if (cudaMallocHost((void**)&t->h_counters, 2 * sizeof(uint32_t)) != cudaSuccess) {
-        cudaGetLastError(); famsa_tree_free(t); set_error("famsa_tree_create: pinned allocation failed"); return FAMSA_ENOMEM;
+    TREE_TRY(tree_alloc(&t->pick, n)); TREE_TRY(tree_alloc(&t->bparent, n)); TREE_TRY(tree_alloc(&t->rootidx, n)); TREE_TRY(tree_alloc(&t->cid16, n));
+    TREE_TRY(tree_alloc(&t->ktab, (size_t)std::min<int64_t>(std::max<int64_t>(k, 1), TREE_SUB_ROWS) * KSTRIDE));
+    TREE_TRY(tree_alloc(&t->wab, (size_t)KSTRIDE * KSTRIDE));
+    t->s_cap = n + (size_t)std::min<int64_t>(std::max<int64_t>(k, 1), TREE_SUB_ROWS) * KSTRIDE;
+    TREE_TRY(tree_alloc(&t->sa, t->s_cap)); TREE_TRY(tree_alloc(&t->sb, t->s_cap)); TREE_TRY(tree_alloc(&t->sw, t->s_cap));
+    TREE_TRY(tree_alloc(&t->st, 1));
+    if (cudaMemset(t->st, 0, sizeof(TreeState)) != cudaSuccess || cudaMallocHost((void**)&t->h_st, sizeof(TreeState)) != cudaSuccess) {
+        cudaGetLastError(); famsa_tree_free(t); set_error("famsa_tree_create: state allocation failed"); return FAMSA_ENOMEM;
     }
     *out = t;
     return FAMSA_OK;
 }
-
-namespace famsa {
-
-// Boruvka rounds over (current forest) + (dense block rows [i0, i1), if any) + (xm extra edges).
-static int tree_rounds(famsa_tree* t, int64_t i0, int64_t i1, const float* sim_block,
-                       const uint32_t* xa, const uint32_t* xb, const float* xw, uint32_t xm, cudaStream_t st) {
-    const int cur = t->cur, nxt = cur ^ 1;
-    TreeArgs a;
-    a.n = (uint32_t)t->k; a.i0 = (uint32_t)i0; a.i1 = (uint32_t)i1; a.m = (uint32_t)t->m;
-    a.xa = xa; a.xb = xb; a.xw = xw; a.xm = xm;
-    a.ta = t->ta[cur]; a.tb = t->tb[cur]; a.tw = t->tw[cur];
-    a.na = t->ta[nxt]; a.nb = t->tb[nxt]; a.nw = t->tw[nxt];
-    a.parent = t->parent;
-    a.cw_row = t->cand_w[0]; a.co_row = t->cand_o[0]; a.cw_col = t->cand_w[1]; a.co_col = t->cand_o[1];
-    a.best_w = t->best_w; a.best_id = t->best_id; a.counters = t->counters;
-    const bool dense = i1 > i0 && i1 >= 2;
-    const int64_t out_base = i0 * (i0 - 1) / 2;
-    const unsigned gv = (unsigned)((a.n + 255) / 256);
-    const unsigned gi = (unsigned)((2ull * a.n + a.m + a.xm + 255) / 256);
-    // a dense row v links every u < v, so after any dense update leaves 0..max_row_end-1 are ONE component
-    // and the leaves above are singletons: the round that reaches that count is the last one.  Without a
-    // dense block (merge of sparse edges) the loop ends on the first round that hooks nothing.
-    const int64_t max_end = std::max<int64_t>(t->max_row_end, dense ? i1 : 0);
-    const uint32_t roots_done = max_end >= 2 ? (uint32_t)(1 + t->k - max_end) : (uint32_t)t->k;
-    int cb = 0;                                            // which comp buffer holds the current labels
-    uint32_t hooked = 0;
-    for (int round = 0; round < 64; ++round) {
-        a.comp = t->comp[cb]; a.comp_next = t->comp[cb ^ 1];
-        tree_reset_kernel<<<gv, 256, 0, st>>>(a, round == 0);
-        if (dense) {
-            tree_row_kernel<1><<<(unsigned)(i1 - i0), 256, 0, st>>>(sim_block, a.i0, a.i1, out_base, a.comp, t->cand_w[0], t->cand_o[0]);
-            tree_col_kernel<<<(unsigned)((a.i1 - 1 + COL_X - 1) / COL_X), dim3(COL_X, COL_Y), 0, st>>>(sim_block, a.i0, a.i1, out_base, a.comp, t->cand_w[1], t->cand_o[1]);
-            t->launches += 2;
-        }
-        tree_best_kernel<0><<<gi, 256, 0, st>>>(a);
-        tree_best_kernel<1><<<gi, 256, 0, st>>>(a);
-        tree_hook_kernel<<<gv, 256, 0, st>>>(a);
-        tree_relabel_kernel<<<gv, 256, 0, st>>>(a);
-        FAMSA_CUDA(cudaMemcpyAsync(t->h_counters, t->counters, 2 * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
-        FAMSA_CUDA(cudaStreamSynchronize(st));
-        t->launches += 5; t->rounds++;
-        cb ^= 1;
-        const bool progress = t->h_counters[0] != hooked;
-        hooked = t->h_counters[0];
-        if (!progress || (!t->merged && xm == 0 && t->h_counters[1] == roots_done)) break;
-    }
-    FAMSA_CUDA(cudaGetLastError());
-    if (hooked + t->h_counters[1] != (uint32_t)t->k || (!t->merged && xm == 0 && t->h_counters[1] != roots_done)) {
-        set_error("famsa_tree: Boruvka did not converge (NaN similarities?)"); return FAMSA_EINVAL;
-    }
-    t->cur = nxt; t->m = hooked; t->max_row_end = max_end;
-    return FAMSA_OK;
-}
-
-}  // namespace famsa
 
 extern "C" int famsa_tree_update(famsa_tree* t, int64_t i0, int64_t i1, const float* sim_block, void* cuda_stream) {
     if (!t) { set_error("famsa_tree_update: tree is NULL"); return FAMSA_EINVAL; }
@@ -358,8 +487,11 @@ extern "C" int famsa_tree_update(famsa_tree* t, int64_t i0, int64_t i1, const fl
     if (i1 == i0) return FAMSA_OK;
     if (!sim_block && famsa_rows_pairs(i0, i1) > 0) { set_error("famsa_tree_update: sim_block is NULL"); return FAMSA_EINVAL; }
     FAMSA_CUDA(cudaSetDevice(t->device));
-    if (famsa_rows_pairs(i0, i1) > 0) {
-        int rc = tree_rounds(t, i0, i1, sim_block, nullptr, nullptr, nullptr, 0, (cudaStream_t)cuda_stream);
+    const int64_t out_base = i0 * (i0 - 1) / 2;
+    for (int64_t s0 = i0; s0 < i1; s0 += TREE_SUB_ROWS) {
+        const int64_t s1 = std::min<int64_t>(s0 + TREE_SUB_ROWS, i1);
+        if (famsa_rows_pairs(s0, s1) == 0) continue;       // row 0 alone: no entries
+        int rc = tree_consume(t, s0, s1, sim_block, out_base, 0, false, (cudaStream_t)cuda_stream);
         if (rc != FAMSA_OK) return rc;
     }
     t->rows += i1 - i0;
@@ -370,41 +502,45 @@ extern "C" int famsa_tree_merge_edges(famsa_tree* t, const int64_t* a_host, cons
     if (!t) { set_error("famsa_tree_merge_edges: tree is NULL"); return FAMSA_EINVAL; }
     if (m < 0 || (m > 0 && (!a_host || !b_host || !sim_host))) { set_error("famsa_tree_merge_edges: null input"); return FAMSA_EINVAL; }
     if (m == 0) return FAMSA_OK;
-    if (m > 0x7FFFFFF0LL) { set_error("famsa_tree_merge_edges: too many edges"); return FAMSA_EINVAL; }
     FAMSA_CUDA(cudaSetDevice(t->device));
-    std::vector<uint32_t> a(m), b(m);
-    for (int64_t e = 0; e < m; ++e) {
-        if (a_host[e] < 0 || a_host[e] >= t->k || b_host[e] < 0 || b_host[e] >= t->k || !(sim_host[e] >= 0.0f) || std::signbit(sim_host[e])) {
-            set_error("famsa_tree_merge_edges: edge " + std::to_string(e) + " has a leaf out of range or a negative (-0.0 included) / NaN similarity");
-            return FAMSA_ERANGE;
+    std::vector<uint32_t> a(std::min<int64_t>(m, (int64_t)t->s_cap)), b(a.size());
+    for (int64_t e0 = 0; e0 < m; e0 += (int64_t)t->s_cap) {                // S-sized slices, merged one after the other
+        const int64_t n = std::min<int64_t>(m - e0, (int64_t)t->s_cap);
+        for (int64_t e = 0; e < n; ++e) {
+            const int64_t x = a_host[e0 + e], y = b_host[e0 + e]; const float w = sim_host[e0 + e];
+            if (x < 0 || x >= t->k || y < 0 || y >= t->k || !(w >= 0.0f) || std::signbit(w)) {
+                set_error("famsa_tree_merge_edges: edge " + std::to_string(e0 + e) + " has a leaf out of range or a negative (-0.0 included) / NaN similarity");
+                return FAMSA_ERANGE;
+            }
+            a[e] = (uint32_t)x; b[e] = (uint32_t)y;
         }
-        a[e] = (uint32_t)a_host[e]; b[e] = (uint32_t)b_host[e];
+        FAMSA_CUDA(cudaDeviceSynchronize());                               // S is free (no update in flight)
+        const uint32_t ns = (uint32_t)n;
+        FAMSA_CUDA(cudaMemcpy(t->sa, a.data(), 4ull * n, cudaMemcpyHostToDevice));
+        FAMSA_CUDA(cudaMemcpy(t->sb, b.data(), 4ull * n, cudaMemcpyHostToDevice));
+        FAMSA_CUDA(cudaMemcpy(t->sw, sim_host + e0, 4ull * n, cudaMemcpyHostToDevice));
+        FAMSA_CUDA(cudaMemcpy(&t->st->ns, &ns, sizeof(ns), cudaMemcpyHostToDevice));
+        int rc = tree_merge(t, nullptr);
+        if (rc != FAMSA_OK) return rc;
+        FAMSA_CUDA(cudaDeviceSynchronize());
     }
-    uint32_t *xa = nullptr, *xb = nullptr; float* xw = nullptr;
-    cudaError_t e1 = cudaMalloc((void**)&xa, 4ull * m), e2 = cudaMalloc((void**)&xb, 4ull * m), e3 = cudaMalloc((void**)&xw, 4ull * m);
-    int rc = FAMSA_OK;
-    if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
-        cudaGetLastError(); set_error("famsa_tree_merge_edges: device allocation failed"); rc = FAMSA_ENOMEM;
-    } else if (cudaMemcpy(xa, a.data(), 4ull * m, cudaMemcpyHostToDevice) != cudaSuccess ||
-               cudaMemcpy(xb, b.data(), 4ull * m, cudaMemcpyHostToDevice) != cudaSuccess ||
-               cudaMemcpy(xw, sim_host, 4ull * m, cudaMemcpyHostToDevice) != cudaSuccess) {
-        rc = famsa::cuda_fail(cudaGetLastError(), "famsa_tree_merge_edges: copy");
-    } else {
-        rc = tree_rounds(t, 0, 0, nullptr, xa, xb, xw, (uint32_t)m, nullptr);
-        if (rc == FAMSA_OK) t->merged = true;
-    }
-    cudaFree(xa); cudaFree(xb); cudaFree(xw);
-    return rc;
+    t->merged = true;
+    return FAMSA_OK;
 }
 
-extern "C" int64_t famsa_tree_edge_count(const famsa_tree* t) { return t ? t->m : 0; }
+extern "C" int64_t famsa_tree_edge_count(const famsa_tree* t) {
+    if (!t) return 0;
+    if (tree_read_state(const_cast<famsa_tree*>(t)) != FAMSA_OK) return -1;
+    return t->h_st->m;
+}
 
 extern "C" int famsa_tree_edges(famsa_tree* t, int64_t* a_host, int64_t* b_host, float* sim_host) {
     if (!t) { set_error("famsa_tree_edges: tree is NULL"); return FAMSA_EINVAL; }
-    const int64_t m = t->m;
+    int rc = tree_read_state(t);
+    if (rc != FAMSA_OK) return rc;
+    const int64_t m = t->h_st->m;
     if (m == 0) return FAMSA_OK;
     if (!a_host || !b_host || !sim_host) { set_error("famsa_tree_edges: null output"); return FAMSA_EINVAL; }
-    FAMSA_CUDA(cudaSetDevice(t->device));
     std::vector<uint32_t> a(m), b(m);
     FAMSA_CUDA(cudaMemcpy(a.data(), t->ta[t->cur], sizeof(uint32_t) * m, cudaMemcpyDeviceToHost));
     FAMSA_CUDA(cudaMemcpy(b.data(), t->tb[t->cur], sizeof(uint32_t) * m, cudaMemcpyDeviceToHost));
@@ -425,45 +561,86 @@ __global__ void tree_wkeys_kernel(uint32_t m, const float* tw, const uint32_t* i
     const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
     if (e < m) w_key[e] = ~__float_as_uint(tw[idx[e]]);     // ascending key == descending similarity
 }
+__global__ void tree_uf_init_kernel(uint32_t k, uint32_t* uf, unsigned long long* info) {
+    const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x < k) { uf[x] = x; info[x] = ((unsigned long long)x << 32) | 1u; }   // (cluster id, size)
+}
 
-// The dendrogram from the sorted tree edges: a union-find pass, inherently sequential (O(k alpha(k))
-// L2-resident steps, once per tree).  One warp: all lanes stage a batch of edges in shared memory and
-// write the batch's merges back (coalesced), lane 0 runs the union-find of the batch in between, so the
-// serial path touches global memory only for the union-find arrays themselves.
-constexpr int DG_BATCH = 1024;
-__global__ void __launch_bounds__(32) tree_dendrogram_kernel(uint32_t k, const uint32_t* order, const uint32_t* ta, const uint32_t* tb, const float* tw,
-                                                             uint32_t* uf, long long* cid, long long* csize,
-                                                             long long* out_a, long long* out_b, float* out_w, long long* out_size) {
-    __shared__ uint32_t sa[DG_BATCH], sb[DG_BATCH];
-    __shared__ long long oa[DG_BATCH], ob[DG_BATCH], os[DG_BATCH];
-    const uint32_t lane = threadIdx.x, m = k - 1;
-    for (uint32_t x = lane; x < k; x += 32) { uf[x] = x; cid[x] = x; csize[x] = 1; }
-    __syncwarp();
-    for (uint32_t t0 = 0; t0 < m; t0 += DG_BATCH) {
-        const uint32_t nb = min((uint32_t)DG_BATCH, m - t0);
-        for (uint32_t q = lane; q < nb; q += 32) {
-            const uint32_t e = order[t0 + q];
-            sa[q] = ta[e]; sb[q] = tb[e]; out_w[t0 + q] = tw[e];
+// The dendrogram from the sorted tree edges: Kruskal's union-find in edge order, which is sequential in the
+// unions but not in the memory latency.  One CTA works through the edges in batches of DG_B:
+//   A (all threads)  the roots of both endpoints of the batch's edges, found in the union-find as it stood
+//                    before the batch (read-only walks, all in flight at once: the L2 latency of the finds,
+//                    which made the one-lane version 0.8 us per merge, is paid once per batch);
+//   B (all threads)  equal roots among the 2 x DG_B slots are identified (canonical slot = first occurrence);
+//   C (one thread)   the batch's unions in edge order on a LOCAL union-find over the slots, in shared memory;
+//   D (all threads)  the local result goes back to the global arrays: every root of the batch points to its
+//                    final root, the final roots carry (cluster id, size), the endpoints are compressed.
+// Cluster ids and sizes are < 2^32 (k <= 2^31 - 16), so (id, size) is one 64-bit word.
+constexpr int DG_B = 128;
+__global__ void __launch_bounds__(DG_B) tree_dendrogram_kernel(uint32_t k, const uint32_t* __restrict__ order, const uint32_t* __restrict__ ta,
+                                                               const uint32_t* __restrict__ tb, const float* __restrict__ tw,
+                                                               uint32_t* uf, unsigned long long* info,
+                                                               long long* out_a, long long* out_b, float* out_w, long long* out_size) {
+    __shared__ uint32_t s_root[2 * DG_B];                  // global root of each slot (2q, 2q+1 = the endpoints of edge q)
+    __shared__ uint32_t s_vert[2 * DG_B];                  // the endpoints themselves
+    __shared__ uint16_t s_canon[2 * DG_B];                 // first slot with the same root
+    __shared__ uint16_t s_par[2 * DG_B];                   // local union-find over canonical slots
+    __shared__ unsigned long long s_info[2 * DG_B];        // (cluster id << 32 | size) of a local root
+    const uint32_t tid = threadIdx.x, m = k - 1;
+    for (uint32_t t0 = 0; t0 < m; t0 += DG_B) {
+        const uint32_t nb = min((uint32_t)DG_B, m - t0);
+        // A: roots as of the start of the batch
+        if (tid < nb) {
+            const uint32_t e = order[t0 + tid];
+            out_w[t0 + tid] = tw[e];
+            uint32_t x = ta[e], y = tb[e];
+            s_vert[2 * tid] = x; s_vert[2 * tid + 1] = y;
+            uint32_t px = __ldcg(uf + x), py = __ldcg(uf + y);
+            while (px != x || py != y) {                   // the two walks advance together
+                if (px != x) { x = px; px = __ldcg(uf + x); }
+                if (py != y) { y = py; py = __ldcg(uf + y); }
+            }
+            s_root[2 * tid] = x; s_root[2 * tid + 1] = y;
         }
-        __syncwarp();
-        if (lane == 0) {
+        __syncthreads();
+        // B: canonical slots; the canonical ones load their root's (id, size)
+        for (uint32_t s = tid; s < 2 * nb; s += DG_B) {
+            const uint32_t r = s_root[s];
+            uint32_t c = 0;
+            while (s_root[c] != r) ++c;                    // ends at c == s at the latest
+            s_canon[s] = (uint16_t)c;
+            s_par[s] = (uint16_t)s;
+            if (c == s) s_info[s] = __ldcg(info + r);
+        }
+        __syncthreads();
+        // C: the unions, in edge order
+        if (tid == 0) {
             for (uint32_t q = 0; q < nb; ++q) {
-                uint32_t ra = sa[q], rb = sb[q];
-                uint32_t pa = uf[ra], pb = uf[rb];                  // the two finds advance together
-                while (pa != ra || pb != rb) {
-                    if (pa != ra) { const uint32_t g = uf[pa]; uf[ra] = g; ra = g; pa = uf[ra]; }
-                    if (pb != rb) { const uint32_t g = uf[pb]; uf[rb] = g; rb = g; pb = uf[rb]; }
-                }
-                const long long ia = cid[ra], ib = cid[rb];
-                const long long za = csize[ra], zb = csize[rb];
-                oa[q] = ia < ib ? ia : ib; ob[q] = ia < ib ? ib : ia; os[q] = za + zb;
-                if (za < zb) { const uint32_t s = ra; ra = rb; rb = s; }
-                uf[rb] = ra; csize[ra] = za + zb; cid[ra] = (long long)k + t0 + q;
+                uint32_t x = s_canon[2 * q], y = s_canon[2 * q + 1];
+                while (s_par[x] != x) { s_par[x] = s_par[s_par[x]]; x = s_par[x]; }
+                while (s_par[y] != y) { s_par[y] = s_par[s_par[y]]; y = s_par[y]; }
+                const unsigned long long ix = s_info[x], iy = s_info[y];
+                const long long ia = (long long)(ix >> 32), ib = (long long)(iy >> 32);
+                const unsigned long long sz = (ix & 0xFFFFFFFFull) + (iy & 0xFFFFFFFFull);
+                out_a[t0 + q] = ia < ib ? ia : ib; out_b[t0 + q] = ia < ib ? ib : ia; out_size[t0 + q] = (long long)sz;
+                if ((uint32_t)ix < (uint32_t)iy) { const uint32_t s = x; x = y; y = s; }     // the larger set stays the root
+                s_par[y] = (uint16_t)x;
+                s_info[x] = ((unsigned long long)(k + t0 + q) << 32) | sz;
             }
         }
-        __syncwarp();
-        for (uint32_t q = lane; q < nb; q += 32) { out_a[t0 + q] = oa[q]; out_b[t0 + q] = ob[q]; out_size[t0 + q] = os[q]; }
-        __syncwarp();
+        __syncthreads();
+        // D: back to the global union-find
+        for (uint32_t s = tid; s < 2 * nb; s += DG_B) {
+            uint32_t f = s_canon[s];
+            while (s_par[f] != f) f = s_par[f];            // read-only walk
+            const uint32_t rf = s_root[f];
+            if (s_canon[s] == s) {
+                uf[s_root[s]] = rf;
+                if (f == s) info[rf] = s_info[s];
+            }
+            uf[s_vert[s]] = rf;                            // full compression of the queried leaves
+        }
+        __syncthreads();
     }
 }
 
@@ -472,35 +649,41 @@ __global__ void __launch_bounds__(32) tree_dendrogram_kernel(uint32_t k, const u
 extern "C" int famsa_tree_finish(famsa_tree* t, int64_t* id_a_host, int64_t* id_b_host, float* sim_host, int64_t* size_host) {
     if (!t) { set_error("famsa_tree_finish: tree is NULL"); return FAMSA_EINVAL; }
     if (t->k < 2) return FAMSA_OK;
-    if (t->m != t->k - 1 || (!t->merged && t->rows < t->k)) {
-        set_error("famsa_tree_finish: the forest has " + std::to_string(t->m) + " of " + std::to_string(t->k - 1) +
+    int rc = tree_read_state(t);
+    if (rc != FAMSA_OK) return rc;
+    if ((int64_t)t->h_st->m != t->k - 1 || (!t->merged && t->rows < t->k)) {
+        set_error("famsa_tree_finish: the forest has " + std::to_string(t->h_st->m) + " of " + std::to_string(t->k - 1) +
                   " edges: not every row has been consumed or merged in"); return FAMSA_ERANGE;
     }
     if (!id_a_host || !id_b_host || !sim_host || !size_host) { set_error("famsa_tree_finish: null output"); return FAMSA_EINVAL; }
-    FAMSA_CUDA(cudaSetDevice(t->device));
     const uint32_t k = (uint32_t)t->k, m = k - 1;
     const int cur = t->cur;
-    struct Tmp { std::vector<void*> p; ~Tmp() { for (void* q : p) cudaFree(q); } } tmp;
-    auto dalloc = [&](void** p, size_t bytes) { cudaError_t e = cudaMalloc(p, std::max<size_t>(bytes, 16)); if (e == cudaSuccess) tmp.p.push_back(*p); return e; };
-    unsigned long long *idk = nullptr, *idk2 = nullptr; uint32_t *wk = nullptr, *wk2 = nullptr, *idx = nullptr, *idx2 = nullptr, *order = nullptr, *uf = nullptr;
-    long long *cid = nullptr, *csize = nullptr, *oa = nullptr, *ob = nullptr, *osz = nullptr; float* ow = nullptr; void* cubtmp = nullptr;
-    FAMSA_CUDA(dalloc((void**)&idk, 8ull * m)); FAMSA_CUDA(dalloc((void**)&idk2, 8ull * m));
-    FAMSA_CUDA(dalloc((void**)&wk, 4ull * m)); FAMSA_CUDA(dalloc((void**)&wk2, 4ull * m));
-    FAMSA_CUDA(dalloc((void**)&idx, 4ull * m)); FAMSA_CUDA(dalloc((void**)&idx2, 4ull * m)); FAMSA_CUDA(dalloc((void**)&order, 4ull * m));
-    FAMSA_CUDA(dalloc((void**)&uf, 4ull * k)); FAMSA_CUDA(dalloc((void**)&cid, 8ull * k)); FAMSA_CUDA(dalloc((void**)&csize, 8ull * k));
-    FAMSA_CUDA(dalloc((void**)&oa, 8ull * m)); FAMSA_CUDA(dalloc((void**)&ob, 8ull * m)); FAMSA_CUDA(dalloc((void**)&osz, 8ull * m));
-    FAMSA_CUDA(dalloc((void**)&ow, 4ull * m));
+    // one scratch allocation, carved up (256-byte aligned pieces)
+    size_t off = 0;
+    auto carve = [&](size_t bytes) { const size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
+    size_t b1 = 0, b2 = 0;
+    FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, b1, (unsigned long long*)nullptr, (unsigned long long*)nullptr, (uint32_t*)nullptr, (uint32_t*)nullptr, (int)m));
+    FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, b2, (uint32_t*)nullptr, (uint32_t*)nullptr, (uint32_t*)nullptr, (uint32_t*)nullptr, (int)m));
+    const size_t o_idk = carve(8ull * m), o_idk2 = carve(8ull * m), o_wk = carve(4ull * m), o_wk2 = carve(4ull * m);
+    const size_t o_idx = carve(4ull * m), o_idx2 = carve(4ull * m), o_order = carve(4ull * m), o_uf = carve(4ull * k), o_info = carve(8ull * k);
+    const size_t o_oa = carve(8ull * m), o_ob = carve(8ull * m), o_osz = carve(8ull * m), o_ow = carve(4ull * m), o_cub = carve(std::max(b1, b2));
+    uint8_t* base = nullptr;
+    if (cudaMalloc((void**)&base, off) != cudaSuccess) { cudaGetLastError(); set_error("famsa_tree_finish: device allocation failed"); return FAMSA_ENOMEM; }
+    struct Guard { uint8_t* p; ~Guard() { cudaFree(p); } } guard{base};
+    unsigned long long *idk = (unsigned long long*)(base + o_idk), *idk2 = (unsigned long long*)(base + o_idk2), *info = (unsigned long long*)(base + o_info);
+    uint32_t *wk = (uint32_t*)(base + o_wk), *wk2 = (uint32_t*)(base + o_wk2), *idx = (uint32_t*)(base + o_idx), *idx2 = (uint32_t*)(base + o_idx2);
+    uint32_t *order = (uint32_t*)(base + o_order), *uf = (uint32_t*)(base + o_uf);
+    long long *oa = (long long*)(base + o_oa), *ob = (long long*)(base + o_ob), *osz = (long long*)(base + o_osz);
+    float* ow = (float*)(base + o_ow);
+    void* cubtmp = base + o_cub;
     const unsigned g = (m + 255) / 256;
     tree_sortkeys_kernel<<<g, 256>>>(m, t->ta[cur], t->tb[cur], idk, idx);
-    size_t b1 = 0, b2 = 0;                                  // two stable passes: by edge id, then by similarity
-    FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, b1, idk, idk2, idx, idx2, (int)m));
-    FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, b2, wk, wk2, idx2, order, (int)m));
-    FAMSA_CUDA(dalloc(&cubtmp, std::max(b1, b2)));
-    FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(cubtmp, b1, idk, idk2, idx, idx2, (int)m));
+    FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(cubtmp, b1, idk, idk2, idx, idx2, (int)m));      // two stable passes: by edge id,
     tree_wkeys_kernel<<<g, 256>>>(m, t->tw[cur], idx2, wk);
-    FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(cubtmp, b2, wk, wk2, idx2, order, (int)m));
-    tree_dendrogram_kernel<<<1, 32>>>(k, order, t->ta[cur], t->tb[cur], t->tw[cur], uf, cid, csize, oa, ob, ow, osz);
-    t->launches += 9;
+    FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(cubtmp, b2, wk, wk2, idx2, order, (int)m));       // then by similarity
+    tree_uf_init_kernel<<<(k + 255) / 256, 256>>>(k, uf, info);
+    tree_dendrogram_kernel<<<1, DG_B>>>(k, order, t->ta[cur], t->tb[cur], t->tw[cur], uf, info, oa, ob, ow, osz);
+    t->launches += 10;
     FAMSA_CUDA(cudaGetLastError());
     static_assert(sizeof(long long) == sizeof(int64_t), "int64_t");
     FAMSA_CUDA(cudaMemcpy(id_a_host, oa, 8ull * m, cudaMemcpyDeviceToHost));
@@ -515,7 +698,8 @@ extern "C" int famsa_guide_forest(famsa_ctx* ctx, int64_t block_rows, int64_t pa
     *out = nullptr;
     if (!ctx) { set_error("famsa_guide_forest: ctx is NULL"); return FAMSA_EINVAL; }
     if (block_rows < 0 || parts < 1 || part < 0 || part >= parts) { set_error("famsa_guide_forest: bad block_rows / part / parts"); return FAMSA_EINVAL; }
-    if (block_rows == 0) block_rows = 1024;
+    if (block_rows == 0) block_rows = TREE_SUB_ROWS;
+    if (block_rows > TREE_SUB_ROWS) { set_error("famsa_guide_forest: block_rows must be <= 1024"); return FAMSA_EINVAL; }
     const int64_t k = ctx->k;
     FAMSA_CUDA(cudaSetDevice(ctx->device));
     famsa_tree* t = nullptr;
@@ -532,14 +716,13 @@ extern "C" int famsa_guide_forest(famsa_ctx* ctx, int64_t block_rows, int64_t pa
     for (int64_t n = 0; n < nb; ++n) { rows_of(n, i0, i1); max_pairs = std::max(max_pairs, famsa_rows_pairs(i0, i1)); }
     float* buf[2] = {nullptr, nullptr};
     cudaStream_t sa = nullptr, sb = nullptr;
-    cudaEvent_t ev[2] = {nullptr, nullptr};
+    cudaEvent_t ev_swept[2] = {nullptr, nullptr}, ev_merged[2] = {nullptr, nullptr};
     auto cleanup = [&](bool keep_tree) {
         cudaDeviceSynchronize();
         cudaFree(buf[0]); cudaFree(buf[1]);
         if (sa) cudaStreamDestroy(sa);
         if (sb) cudaStreamDestroy(sb);
-        if (ev[0]) cudaEventDestroy(ev[0]);
-        if (ev[1]) cudaEventDestroy(ev[1]);
+        for (int q = 0; q < 2; ++q) { if (ev_swept[q]) cudaEventDestroy(ev_swept[q]); if (ev_merged[q]) cudaEventDestroy(ev_merged[q]); }
         if (!keep_tree) famsa_tree_free(t);
     };
 #define GT_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { int r__ = (e__ == cudaErrorMemoryAllocation) ? FAMSA_ENOMEM : FAMSA_ECUDA; \
@@ -547,26 +730,34 @@ extern "C" int famsa_guide_forest(famsa_ctx* ctx, int64_t block_rows, int64_t pa
 #define GT_TRY(x) do { int r__ = (x); if (r__ != FAMSA_OK) { cleanup(false); return r__; } } while (0)
     GT_CUDA(cudaMalloc((void**)&buf[0], std::max<int64_t>(max_pairs, 1) * sizeof(float)));
     GT_CUDA(cudaMalloc((void**)&buf[1], std::max<int64_t>(max_pairs, 1) * sizeof(float)));
-    GT_CUDA(cudaStreamCreateWithFlags(&sa, cudaStreamNonBlocking));
-    GT_CUDA(cudaStreamCreateWithFlags(&sb, cudaStreamNonBlocking));
-    GT_CUDA(cudaEventCreateWithFlags(&ev[0], cudaEventDisableTiming));
-    GT_CUDA(cudaEventCreateWithFlags(&ev[1], cudaEventDisableTiming));
-    rows_of(0, i0, i1);
-    if (famsa_rows_pairs(i0, i1) > 0) GT_TRY(famsa::sweep_rows(ctx, i0, i1, nullptr, buf[0], nullptr, sa));
-    GT_CUDA(cudaEventRecord(ev[0], sa));
-    for (int64_t n = 0; n < nb; ++n) {
-        if (n + 1 < nb) {                                  // sweep the next block while this one is merged
-            int64_t n0, n1;
-            rows_of(n + 1, n0, n1);
-            GT_TRY(famsa::sweep_rows(ctx, n0, n1, nullptr, buf[(n + 1) & 1], nullptr, sa));
-            GT_CUDA(cudaEventRecord(ev[(n + 1) & 1], sa));
-        }
-        rows_of(n, i0, i1);
-        GT_CUDA(cudaStreamWaitEvent(sb, ev[n & 1], 0));
-        GT_TRY(famsa_tree_update(t, i0, i1, buf[n & 1], sb));
+    int prio_lo = 0, prio_hi = 0;
+    GT_CUDA(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+    GT_CUDA(cudaStreamCreateWithPriority(&sa, cudaStreamNonBlocking, prio_lo));
+    GT_CUDA(cudaStreamCreateWithPriority(&sb, cudaStreamNonBlocking, prio_hi));   // the tree's small kernels go first when SM resources free up
+    for (int q = 0; q < 2; ++q) {
+        GT_CUDA(cudaEventCreateWithFlags(&ev_swept[q], cudaEventDisableTiming));
+        GT_CUDA(cudaEventCreateWithFlags(&ev_merged[q], cudaEventDisableTiming));
     }
-    ctx->launches += t->launches;
+    // Pipeline, all enqueued without a host round trip: stream sa sweeps block n into buffer n & 1 (its epilogue
+    // also leaves the round-0 candidates in candidate slot n & 1), stream sb merges block n into the forest;
+    // the sweep of block n + 2 waits for the merge of block n (same buffer and slot).
+    for (int64_t n = 0; n < nb; ++n) {
+        const int q = (int)(n & 1);
+        rows_of(n, i0, i1);
+        if (n >= 2) GT_CUDA(cudaStreamWaitEvent(sa, ev_merged[q], 0));
+        if (famsa_rows_pairs(i0, i1) > 0) {
+            GT_TRY(famsa::tree_fused_begin(t, i0, i1, q, sa));
+            famsa::TreeCand tc{t->cand_row[q], t->cand_col[q]};
+            GT_TRY(famsa::sweep_rows(ctx, i0, i1, nullptr, buf[q], nullptr, &tc, sa));
+        }
+        GT_CUDA(cudaEventRecord(ev_swept[q], sa));
+        GT_CUDA(cudaStreamWaitEvent(sb, ev_swept[q], 0));
+        if (famsa_rows_pairs(i0, i1) > 0) GT_TRY(famsa::tree_consume(t, i0, i1, buf[q], i0 * (i0 - 1) / 2, q, true, sb));
+        t->rows += i1 - i0;
+        GT_CUDA(cudaEventRecord(ev_merged[q], sb));
+    }
     cleanup(true);
+    ctx->launches += t->launches;
     *out = t;
     return FAMSA_OK;
 #undef GT_CUDA

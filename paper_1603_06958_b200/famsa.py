@@ -361,6 +361,7 @@ def famsa_tree_update(tree, i0, i1, sim_block, cuda_stream=None):
         assert sim_block.numel() >= famsa_rows_pairs(i0, i1)
     _check(lib().famsa_tree_update(tree.handle, int(i0), int(i1), _ptr(sim_block), cuda_stream))
     tree.rows += int(i1) - int(i0)
+    tree._last_block = sim_block          # the call only enqueues: keep the block alive until the next one / a query
 
 
 def famsa_tree_merge_edges(tree, a, b, sim):
