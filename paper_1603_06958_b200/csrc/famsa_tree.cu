@@ -570,30 +570,37 @@ __global__ void tree_uf_init_kernel(uint32_t k, uint32_t* uf, unsigned long long
 // unions but not in the memory latency.  One CTA works through the edges in batches of DG_B:
 //   A (all threads)  the roots of both endpoints of the batch's edges, found in the union-find as it stood
 //                    before the batch (read-only walks, all in flight at once: the L2 latency of the finds,
-//                    which made the one-lane version 0.8 us per merge, is paid once per batch);
-//   B (all threads)  equal roots among the 2 x DG_B slots are identified (canonical slot = first occurrence);
-//   C (one thread)   the batch's unions in edge order on a LOCAL union-find over the slots, in shared memory;
+//                    which made the one-lane version 0.8 us per merge, is paid once per batch; the endpoints
+//                    of the NEXT batch are fetched before this batch's serial phase);
+//   B (all threads)  equal roots among the 2 x DG_B slots are identified through a small shared-memory hash
+//                    table (canonical slot = smallest slot with that root);
+//   C (one thread)   the batch's unions in edge order on a LOCAL union-find over the slots, in shared memory,
+//                    with the next edge's slots and the (speculative) set records loaded ahead;
 //   D (all threads)  the local result goes back to the global arrays: every root of the batch points to its
 //                    final root, the final roots carry (cluster id, size), the endpoints are compressed.
 // Cluster ids and sizes are < 2^32 (k <= 2^31 - 16), so (id, size) is one 64-bit word.
-constexpr int DG_B = 128;
+constexpr int DG_B = 128, DG_H = 512;
 __global__ void __launch_bounds__(DG_B) tree_dendrogram_kernel(uint32_t k, const uint32_t* __restrict__ order, const uint32_t* __restrict__ ta,
                                                                const uint32_t* __restrict__ tb, const float* __restrict__ tw,
                                                                uint32_t* uf, unsigned long long* info,
                                                                long long* out_a, long long* out_b, float* out_w, long long* out_size) {
     __shared__ uint32_t s_root[2 * DG_B];                  // global root of each slot (2q, 2q+1 = the endpoints of edge q)
     __shared__ uint32_t s_vert[2 * DG_B];                  // the endpoints themselves
-    __shared__ uint16_t s_canon[2 * DG_B];                 // first slot with the same root
+    __shared__ __align__(4) uint16_t s_canon[2 * DG_B + 2];   // smallest slot with the same root (+2: read-ahead slack)
     __shared__ uint16_t s_par[2 * DG_B];                   // local union-find over canonical slots
+    __shared__ uint16_t s_hidx[2 * DG_B];
     __shared__ unsigned long long s_info[2 * DG_B];        // (cluster id << 32 | size) of a local root
+    __shared__ uint32_t h_key[DG_H], h_slot[DG_H];
     const uint32_t tid = threadIdx.x, m = k - 1;
+    uint32_t nx = 0, ny = 0; float nw = 0.0f;              // this thread's edge of the next batch
+    if (tid < m) { const uint32_t e = order[tid]; nx = ta[e]; ny = tb[e]; nw = tw[e]; }
     for (uint32_t t0 = 0; t0 < m; t0 += DG_B) {
         const uint32_t nb = min((uint32_t)DG_B, m - t0);
+        for (uint32_t h = tid; h < DG_H; h += DG_B) { h_key[h] = 0xFFFFFFFFu; h_slot[h] = 0xFFFFFFFFu; }
         // A: roots as of the start of the batch
         if (tid < nb) {
-            const uint32_t e = order[t0 + tid];
-            out_w[t0 + tid] = tw[e];
-            uint32_t x = ta[e], y = tb[e];
+            uint32_t x = nx, y = ny;
+            out_w[t0 + tid] = nw;
             s_vert[2 * tid] = x; s_vert[2 * tid + 1] = y;
             uint32_t px = __ldcg(uf + x), py = __ldcg(uf + y);
             while (px != x || py != y) {                   // the two walks advance together
@@ -602,30 +609,47 @@ __global__ void __launch_bounds__(DG_B) tree_dendrogram_kernel(uint32_t k, const
             }
             s_root[2 * tid] = x; s_root[2 * tid + 1] = y;
         }
+        if (t0 + DG_B + tid < m) { const uint32_t e = order[t0 + DG_B + tid]; nx = ta[e]; ny = tb[e]; nw = tw[e]; }   // in flight during B-D
         __syncthreads();
-        // B: canonical slots; the canonical ones load their root's (id, size)
+        // B: canonical slots through the hash table; the canonical ones load their root's (id, size)
         for (uint32_t s = tid; s < 2 * nb; s += DG_B) {
             const uint32_t r = s_root[s];
-            uint32_t c = 0;
-            while (s_root[c] != r) ++c;                    // ends at c == s at the latest
-            s_canon[s] = (uint16_t)c;
+            uint32_t h = (r * 2654435761u) >> 23;           // 9 bits
+            for (;;) {
+                const uint32_t old = atomicCAS(&h_key[h], 0xFFFFFFFFu, r);
+                if (old == 0xFFFFFFFFu || old == r) break;
+                h = (h + 1) & (DG_H - 1);
+            }
+            atomicMin(&h_slot[h], s);
+            s_hidx[s] = (uint16_t)h;
             s_par[s] = (uint16_t)s;
-            if (c == s) s_info[s] = __ldcg(info + r);
+        }
+        __syncthreads();
+        for (uint32_t s = tid; s < 2 * nb; s += DG_B) {
+            const uint32_t c = h_slot[s_hidx[s]];
+            s_canon[s] = (uint16_t)c;
+            if (c == s) s_info[s] = __ldcg(info + s_root[s]);
         }
         __syncthreads();
         // C: the unions, in edge order
         if (tid == 0) {
+            const uint32_t* canon2 = reinterpret_cast<const uint32_t*>(s_canon);
+            uint32_t cc = canon2[0];
             for (uint32_t q = 0; q < nb; ++q) {
-                uint32_t x = s_canon[2 * q], y = s_canon[2 * q + 1];
-                while (s_par[x] != x) { s_par[x] = s_par[s_par[x]]; x = s_par[x]; }
-                while (s_par[y] != y) { s_par[y] = s_par[s_par[y]]; y = s_par[y]; }
-                const unsigned long long ix = s_info[x], iy = s_info[y];
+                const uint32_t cnext = canon2[q + 1];      // read ahead (slack entry past the batch)
+                uint32_t x = cc & 0xFFFFu, y = cc >> 16;
+                uint32_t px = s_par[x], py = s_par[y];
+                unsigned long long ix = s_info[x], iy = s_info[y];   // valid if x, y are local roots (the common case)
+                if (px != x) { do { x = px; px = s_par[x]; } while (px != x); ix = s_info[x]; }
+                if (py != y) { do { y = py; py = s_par[y]; } while (py != y); iy = s_info[y]; }
                 const long long ia = (long long)(ix >> 32), ib = (long long)(iy >> 32);
                 const unsigned long long sz = (ix & 0xFFFFFFFFull) + (iy & 0xFFFFFFFFull);
                 out_a[t0 + q] = ia < ib ? ia : ib; out_b[t0 + q] = ia < ib ? ib : ia; out_size[t0 + q] = (long long)sz;
                 if ((uint32_t)ix < (uint32_t)iy) { const uint32_t s = x; x = y; y = s; }     // the larger set stays the root
                 s_par[y] = (uint16_t)x;
+                s_par[cc & 0xFFFFu] = (uint16_t)x; s_par[cc >> 16] = (uint16_t)x;            // compress both starting slots
                 s_info[x] = ((unsigned long long)(k + t0 + q) << 32) | sz;
+                cc = cnext;
             }
         }
         __syncthreads();
