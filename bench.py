@@ -162,6 +162,7 @@ def time_bitparallel(seqs, offsets, blocks, seconds, seed):
     def sample(n_rows):
         ri = rng.choice(rows_all, size=n_rows, p=rows_all / rows_all.sum())
         cj = (rng.random((n_rows, ncol)) * ri[:, None]).astype(np.int64)
+        cj.sort(axis=1)           # sorted indices = sorted lengths: the `a` pairs of one SIMD step have similar lengths
         cells = float((lens[ri][:, None] * lens[cj]).sum())
         col_ptr = np.arange(n_rows + 1, dtype=np.int64) * ncol
         return perm[ri], col_ptr, perm[cj].ravel(), cells

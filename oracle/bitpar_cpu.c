@@ -17,6 +17,9 @@
 #include <stdlib.h>
 #include <string.h>
 #include <pthread.h>
+#if defined(__x86_64__)
+#include <immintrin.h>
+#endif
 
 #define SYMS 32
 #define PAD_SYM 31           /* never a residue code (codes are < 25): its match words are all zero */
@@ -53,7 +56,10 @@ static int32_t lcs_scalar(const uint64_t *M, int32_t W, const uint8_t *b, int32_
 /* SIMD: N pairs (one table, N column sequences) per vector of N 64-bit lanes.  V: N*W words of scratch
  * (vector-aligned).  Columns shorter than the group's longest are padded with PAD_SYM (a no-op step).
  * The body is written once with GCC vector extensions and instantiated per lane count and target ISA. */
-#define DEFINE_LCS_VEC(NAME, N, TARGET)                                                                   \
+/* GATHER(mw, row, sym): lane l of mw = row[sym[l]] -- element-wise for the generic vectors, the hardware    */
+/* gather instruction where the ISA has one.                                                               */
+#define GATHER_GENERIC(N, mw, row, sym) do { int l_; for (l_ = 0; l_ < N; ++l_) (mw)[l_] = (row)[(sym)[l_]]; } while (0)
+#define DEFINE_LCS_VEC(NAME, N, TARGET, GATHER)                                                           \
     typedef uint64_t NAME##_vec __attribute__((vector_size(8 * N)));                                      \
     TARGET static void NAME(const uint64_t *M, int32_t W, const uint8_t *const *b, const int32_t *lb,     \
                             int32_t n, NAME##_vec *V, int32_t *out)                                       \
@@ -63,13 +69,13 @@ static int32_t lcs_scalar(const uint64_t *M, int32_t W, const uint8_t *b, int32_
         for (l = 0; l < n; ++l) if (lb[l] > maxlen) maxlen = lb[l];                                       \
         for (w = 0; w < W; ++w) V[w] = ones;                                                              \
         for (j = 0; j < maxlen; ++j) {                                                                    \
-            uint32_t sym[N];                                                                              \
+            long long sym[N] __attribute__((aligned(64)));                                                \
             NAME##_vec carry = (NAME##_vec){0};                                                           \
             for (l = 0; l < N; ++l) sym[l] = (l < n && j < lb[l]) ? b[l][j] : PAD_SYM;                    \
             for (w = 0; w < W; ++w) {                                                                     \
                 const uint64_t *row = M + (size_t)w * SYMS;                                               \
                 NAME##_vec mw, u, t, s;                                                                   \
-                for (l = 0; l < N; ++l) mw[l] = row[sym[l]];            /* gather: lane l's symbol */      \
+                GATHER(mw, row, sym);                                   /* lane l's symbol */              \
                 u = V[w] & mw;                                                                            \
                 t = V[w] + u;                                                                             \
                 s = t - carry;                                          /* carry is a 0 / -1 lane mask */  \
@@ -84,12 +90,19 @@ static int32_t lcs_scalar(const uint64_t *M, int32_t W, const uint8_t *b, int32_
         }                                                                                                 \
     }
 
-DEFINE_LCS_VEC(lcs_v2, 2, )
-DEFINE_LCS_VEC(lcs_v4, 4, )
-DEFINE_LCS_VEC(lcs_v8, 8, )
+#define GATHER_2(mw, row, sym) GATHER_GENERIC(2, mw, row, sym)
+#define GATHER_4(mw, row, sym) GATHER_GENERIC(4, mw, row, sym)
+#define GATHER_8(mw, row, sym) GATHER_GENERIC(8, mw, row, sym)
+DEFINE_LCS_VEC(lcs_v2, 2, , GATHER_2)
+DEFINE_LCS_VEC(lcs_v4, 4, , GATHER_4)
+DEFINE_LCS_VEC(lcs_v8, 8, , GATHER_8)
 #if defined(__x86_64__)
-DEFINE_LCS_VEC(lcs_v4_avx2, 4, __attribute__((target("avx2"))))
-DEFINE_LCS_VEC(lcs_v8_avx512, 8, __attribute__((target("avx512f,avx512bw,avx512dq,avx512vl"))))
+#define GATHER_AVX2(mw, row, sym) \
+    (mw) = (__typeof__(mw))_mm256_i64gather_epi64((const long long *)(row), _mm256_load_si256((const __m256i *)(sym)), 8)
+#define GATHER_AVX512(mw, row, sym) \
+    (mw) = (__typeof__(mw))_mm512_i64gather_epi64(_mm512_load_si512((const void *)(sym)), (const void *)(row), 8)
+DEFINE_LCS_VEC(lcs_v4_avx2, 4, __attribute__((target("avx2"))), GATHER_AVX2)
+DEFINE_LCS_VEC(lcs_v8_avx512, 8, __attribute__((target("avx512f,avx512bw,avx512dq,avx512vl"))), GATHER_AVX512)
 #endif
 
 /* ISA codes of bitpar_rowsets: 0 scalar; 2 / 4 / 8 generic vectors of that many lanes (compiled for the

@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.environ.get("FAMSA_LIB_OUT") or os.path.join(HERE, "libfamsa_lcs.so")
 OBJ_DIR = os.path.join(HERE, "build")
-SOURCES = ["famsa_pack.cu", "famsa_sweep.cu", "famsa_peak.cu", "famsa_tree.cu"]
+SOURCES = ["famsa_pack.cu", "famsa_sweep.cu", "famsa_peak.cu", "famsa_tree.cu", "famsa_profile.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC] + os.environ.get("FAMSA_NVCC_EXTRA", "").split()

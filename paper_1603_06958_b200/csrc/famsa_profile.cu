@@ -1,0 +1,247 @@
+// famsa_profile.cu -- SURVEY.md 8(f) NEXT-4: sequence-versus-profile dynamic programming of FAMSA's stage III
+// (PAPER.md:71-79, 107, 111-116, 133-139).  Boundary and the readings of the paper: include/famsa_profile.h,
+// DESIGN.md P1-P9.
+//
+// Mapping: one warp per alignment.  The SEQUENCE side (n2 <= 1024 residues) is spread over the 32 lanes, J =
+// 4 / 8 / 16 / 32 consecutive residues per lane, and for each of them the lane keeps the three states of the
+// previous profile column (row) in registers: 3 J floats.  The rows are swept in a skewed wavefront: at step t
+// lane l computes row t - l + 1, so what it needs from the left -- the three states of lane l-1's last residue
+// in the same row -- was produced one step earlier and arrives by one __shfl_up per state; the value received
+// for the previous row is kept as the diagonal.  Per cell: one L1-resident load of cost[row][residue] and ~25
+// fp32 adds / compares / selects, one direction byte (2 bits per state).  All arithmetic is fp32 adds,
+// subtractions and comparisons in the order the oracle's fp32 mode uses (products of nseq and a gap cost are
+// formed once with __fmul_rn, nothing can contract into an FMA), so scores AND traceback decisions are
+// bit-identical to it.  A second kernel (one thread per alignment) walks the direction bytes back.
+#include <algorithm>
+#include <cmath>
+#include <vector>
+
+#include "famsa_internal.h"
+#include "famsa_profile.h"
+
+namespace famsa {
+
+constexpr float NEG = -3.0e38f;
+
+struct AlignDesc {
+    int64_t cost_row0;       // first cost row of the profile
+    int64_t seq0;            // first residue of the sequence
+    int64_t dir0;            // byte offset of the direction matrix in the workspace (row stride 32 J)
+    int64_t path_end;        // end of the path segment
+    int32_t n1, n2, idx, j;  // columns, residues, index in the batch, residues per lane
+};
+
+__global__ void profile_costs_kernel(const uint32_t* __restrict__ counts, const float* __restrict__ subst, int64_t n_cols, float* __restrict__ cost) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_cols * SYMS) return;
+    const int64_t i = t / SYMS; const int c = (int)(t % SYMS);
+    double s = 0.0;
+#pragma unroll 8
+    for (int d = 0; d < SYMS; ++d) s = __dadd_rn(s, __dmul_rn((double)counts[i * SYMS + d], (double)subst[d * SYMS + c]));
+    cost[t] = (float)s;
+}
+
+template <int J>
+__global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restrict__ desc, int n, const float* __restrict__ cost,
+                                                      const uint8_t* __restrict__ seq, const float* __restrict__ gaps,
+                                                      const int32_t* __restrict__ nseq, float* __restrict__ score,
+                                                      uint8_t* __restrict__ final_state, uint8_t* __restrict__ ws, int want_dir) {
+    const int warp = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+    if (warp >= n) return;
+    const AlignDesc d = desc[warp];
+    const int n1 = d.n1, n2 = d.n2, b = d.idx;
+    const float To = gaps[4 * b], Te = gaps[4 * b + 1], Go = gaps[4 * b + 2], Ge = gaps[4 * b + 3];
+    const float ns = (float)nseq[b];
+    const float nTo = __fmul_rn(ns, To), nTe = __fmul_rn(ns, Te), nGo = __fmul_rn(ns, Go), nGe = __fmul_rn(ns, Ge);
+    const int j0 = lane * J;                                 // this lane owns residues j0+1 .. j0+J (1-based)
+    uint32_t yw[J / 4];                                      // their codes, 4 per word (code*4 = byte offset in a cost row)
+#pragma unroll
+    for (int q = 0; q < J / 4; ++q) {
+        uint32_t w = 0;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) { const int jj = j0 + 4 * q + r; w |= (uint32_t)(jj < n2 ? seq[d.seq0 + jj] : 0) << (8 * r); }
+        yw[q] = w;
+    }
+    // row 0: residues before the first column are terminal gap columns, Y[0][j] = Y[0][j-1] - nseq T_e
+    float yrun = 0.0f;
+    for (int j = 1; j <= j0; ++j) yrun = j == 1 ? 0.0f - nTo : yrun - nTe;
+    float dM = lane == 0 ? 0.0f : NEG, dX = NEG, dY = lane == 0 ? NEG : yrun;     // row 0 at residue j0: the first diagonal
+    float Mp[J], Xp[J], Yp[J];
+#pragma unroll
+    for (int c = 0; c < J; ++c) { yrun = (j0 + c + 1) == 1 ? 0.0f - nTo : yrun - nTe; Mp[c] = NEG; Xp[c] = NEG; Yp[c] = yrun; }
+    float x0 = 0.0f;                                         // lane 0: X[i][0], columns before the first residue
+    float rM = NEG, rX = NEG, rY = NEG;                      // the row this lane finished last, at its last residue
+    const float* crow = cost + d.cost_row0 * SYMS;
+    uint8_t* dir = ws + d.dir0;
+    const int stride = 32 * J;
+    const int steps = n1 + 31;
+    for (int t = 0; t < steps; ++t) {
+        const int i = t - lane + 1;
+        float lM = __shfl_up_sync(0xffffffffu, rM, 1), lX = __shfl_up_sync(0xffffffffu, rX, 1), lY = __shfl_up_sync(0xffffffffu, rY, 1);
+        if (i < 1 || i > n1) continue;                       // (no shuffle below this line)
+        if (lane == 0) { x0 = i == 1 ? 0.0f - To : x0 - Te; lM = NEG; lX = x0; lY = NEG; }
+        const float goy = i == n1 ? nTo : nGo, gey = i == n1 ? nTe : nGe;
+        const float* ci = crow + (size_t)(i - 1) * SYMS;
+        float cM = dM, cX = dX, cY = dY;                     // diagonal of the lane's first residue
+        dM = lM; dX = lX; dY = lY;                           // ... and the next row's
+        uint32_t dword = 0;
+#pragma unroll
+        for (int c = 0; c < J; ++c) {
+            const int j = j0 + c + 1;
+            const float gox = j == n2 ? To : Go, gex = j == n2 ? Te : Ge;
+            const uint32_t code = (yw[c >> 2] >> (8 * (c & 3))) & 0xFFu;
+            float bst = cM, v; uint32_t from = 0, dd;
+            if (cX > bst) { bst = cX; from = 1; }
+            if (cY > bst) { bst = cY; from = 2; }
+            const float m = bst + __ldg(ci + code); dd = from;
+            bst = Mp[c] - gox; from = 0;
+            v = Xp[c] - gex; if (v > bst) { bst = v; from = 1; }
+            v = Yp[c] - gox; if (v > bst) { bst = v; from = 2; }
+            const float x = bst; dd |= from << 2;
+            bst = lM - goy; from = 0;
+            v = lX - goy; if (v > bst) { bst = v; from = 1; }
+            v = lY - gey; if (v > bst) { bst = v; from = 2; }
+            const float y = bst; dd |= from << 4;
+            cM = Mp[c]; cX = Xp[c]; cY = Yp[c];
+            Mp[c] = m; Xp[c] = x; Yp[c] = y;
+            lM = m; lX = x; lY = y;
+            dword |= dd << (8 * (c & 3));
+            if ((c & 3) == 3) {
+                if (want_dir) *reinterpret_cast<uint32_t*>(dir + (size_t)(i - 1) * stride + j0 + c - 3) = dword;
+                dword = 0;
+            }
+            if (i == n1 && j == n2) {                        // the end cell: score and the state the walk starts in
+                float best = m; uint32_t st = 0;
+                if (x > best) { best = x; st = 1; }
+                if (y > best) { best = y; st = 2; }
+                score[b] = best; final_state[b] = (uint8_t)st;
+            }
+        }
+        rM = lM; rX = lX; rY = lY;
+    }
+}
+
+// One thread per alignment walks the direction bytes from (n1, n2) back to (0, 0); the operations are written
+// right-aligned into the alignment's path segment.
+__global__ void seqprof_trace_kernel(const AlignDesc* __restrict__ desc, int n, const uint8_t* __restrict__ final_state,
+                                     const uint8_t* __restrict__ ws, uint8_t* __restrict__ path, int32_t* __restrict__ path_len) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const AlignDesc d = desc[t];
+    const uint8_t* dir = ws + d.dir0;
+    const int stride = 32 * d.j;
+    int i = d.n1, j = d.n2, len = 0;
+    uint32_t st = final_state[d.idx];
+    uint8_t* out = path + d.path_end;
+    while (i > 0 || j > 0) {
+        uint32_t dd;
+        if (i > 0 && j > 0) dd = dir[(size_t)(i - 1) * stride + (j - 1)];
+        else if (i == 0) dd = (j == 1 ? 0u : 2u) << 4;        // row 0: a run of terminal gap columns
+        else dd = (i == 1 ? 0u : 1u) << 2;                    // residue 0: a run of terminal gaps
+        *--out = (uint8_t)st; ++len;
+        if (st == 0) { st = dd & 3; --i; --j; }
+        else if (st == 1) { st = (dd >> 2) & 3; --i; }
+        else { st = (dd >> 4) & 3; --j; }
+    }
+    path_len[d.idx] = len;
+}
+
+static int lanes_j(int64_t n2) { return n2 <= 128 ? 4 : (n2 <= 256 ? 8 : (n2 <= 512 ? 16 : 32)); }
+
+}  // namespace famsa
+
+using namespace famsa;
+
+extern "C" double famsa_gap_scale(double k, double g_l, double g_d) { return 1.0 + std::log(k / g_l) / g_d; }
+
+extern "C" int famsa_profile_costs(const uint32_t* counts_dev, const float* subst_dev, int64_t n_cols, float* cost_dev, void* cuda_stream) {
+    if (n_cols < 0 || (n_cols > 0 && (!counts_dev || !subst_dev || !cost_dev))) { set_error("famsa_profile_costs: null pointer or n_cols < 0"); return FAMSA_EINVAL; }
+    if (n_cols == 0) return FAMSA_OK;
+    profile_costs_kernel<<<(unsigned)((n_cols * SYMS + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(counts_dev, subst_dev, n_cols, cost_dev);
+    FAMSA_CUDA(cudaGetLastError());
+    return FAMSA_OK;
+}
+
+static int seqprof_check(const int64_t* col_off, const int64_t* seq_off, int64_t n, const char* who) {
+    if (n < 0 || !col_off || !seq_off) { set_error(std::string(who) + ": null offsets or n_align < 0"); return FAMSA_EINVAL; }
+    if (col_off[0] < 0 || seq_off[0] < 0) { set_error(std::string(who) + ": negative offset"); return FAMSA_EINVAL; }
+    for (int64_t b = 0; b < n; ++b) {
+        const int64_t n1 = col_off[b + 1] - col_off[b], n2 = seq_off[b + 1] - seq_off[b];
+        if (n1 < 1 || n2 < 1 || n2 > FAMSA_SEQPROF_MAX_SEQ || n1 > 0x7FFFFFF0LL) {
+            set_error(std::string(who) + ": alignment " + std::to_string(b) + " has an empty profile, an empty sequence or more than " +
+                      std::to_string(FAMSA_SEQPROF_MAX_SEQ) + " residues");
+            return FAMSA_ELENGTH;
+        }
+    }
+    return FAMSA_OK;
+}
+
+extern "C" int64_t famsa_seqprof_workspace(const int64_t* col_off_host, const int64_t* seq_off_host, int64_t n_align) {
+    if (seqprof_check(col_off_host, seq_off_host, n_align, "famsa_seqprof_workspace") != FAMSA_OK) return -1;
+    int64_t bytes = 0;
+    for (int64_t b = 0; b < n_align; ++b)
+        bytes += (col_off_host[b + 1] - col_off_host[b]) * 32 * lanes_j(seq_off_host[b + 1] - seq_off_host[b]);
+    return bytes + n_align;                                  // + one final-state byte per alignment
+}
+
+extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off_host, const uint8_t* seq_dev,
+                                   const int64_t* seq_off_host, const float* gaps_dev, const int32_t* nseq_dev, int64_t n_align,
+                                   float* score_dev, uint8_t* path_dev, int32_t* path_len_dev, void* workspace_dev, void* cuda_stream) {
+    int rc = seqprof_check(col_off_host, seq_off_host, n_align, "famsa_seqprof_align");
+    if (rc != FAMSA_OK) return rc;
+    if (n_align == 0) return FAMSA_OK;
+    if (n_align > 0x7FFFFFF0LL) { set_error("famsa_seqprof_align: too many alignments"); return FAMSA_EINVAL; }
+    if (!cost_dev || !seq_dev || !gaps_dev || !nseq_dev || !score_dev || (path_dev && (!path_len_dev || !workspace_dev))) {
+        set_error("famsa_seqprof_align: null pointer (path_dev needs path_len_dev and workspace_dev)"); return FAMSA_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // descriptors, grouped by residues-per-lane variant (longest profiles first inside a group: the heavy warps start first)
+    std::vector<AlignDesc> desc((size_t)n_align);
+    std::vector<int64_t> order((size_t)n_align);
+    int64_t dir_bytes = 0;
+    for (int64_t b = 0; b < n_align; ++b) {
+        AlignDesc& d = desc[(size_t)b];
+        d.cost_row0 = col_off_host[b]; d.seq0 = seq_off_host[b];
+        d.n1 = (int32_t)(col_off_host[b + 1] - col_off_host[b]); d.n2 = (int32_t)(seq_off_host[b + 1] - seq_off_host[b]);
+        d.idx = (int32_t)b; d.j = lanes_j(d.n2);
+        d.dir0 = dir_bytes; dir_bytes += (int64_t)d.n1 * 32 * d.j;
+        d.path_end = col_off_host[b + 1] + seq_off_host[b + 1];
+        order[(size_t)b] = b;
+    }
+    std::stable_sort(order.begin(), order.end(), [&](int64_t p, int64_t q) {
+        const AlignDesc &a = desc[(size_t)p], &c = desc[(size_t)q];
+        return a.j != c.j ? a.j < c.j : a.n1 > c.n1;
+    });
+    std::vector<AlignDesc> sorted((size_t)n_align);
+    for (int64_t b = 0; b < n_align; ++b) sorted[(size_t)b] = desc[(size_t)order[(size_t)b]];
+    uint8_t* final_state = nullptr;
+    uint8_t* ws = static_cast<uint8_t*>(workspace_dev);
+    AlignDesc* d_desc = nullptr;
+    uint8_t* own_state = nullptr;
+    FAMSA_CUDA(cudaMallocAsync((void**)&d_desc, sizeof(AlignDesc) * (size_t)n_align, st));
+    if (ws) final_state = ws + dir_bytes;
+    else { FAMSA_CUDA(cudaMallocAsync((void**)&own_state, (size_t)n_align, st)); final_state = own_state; }
+    FAMSA_CUDA(cudaMemcpyAsync(d_desc, sorted.data(), sizeof(AlignDesc) * (size_t)n_align, cudaMemcpyHostToDevice, st));
+    FAMSA_CUDA(cudaStreamSynchronize(st));                   // `sorted` is pageable and dies with this call
+    const int want_dir = path_dev != nullptr;
+    int64_t g0 = 0;
+    while (g0 < n_align) {
+        int64_t g1 = g0;
+        while (g1 < n_align && sorted[(size_t)g1].j == sorted[(size_t)g0].j) ++g1;
+        const int n = (int)(g1 - g0);
+        const unsigned grid = (unsigned)((n + 3) / 4);       // 4 warps = 4 alignments per CTA
+        switch (sorted[(size_t)g0].j) {
+            case 4:  seqprof_kernel<4><<<grid, 128, 0, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
+            case 8:  seqprof_kernel<8><<<grid, 128, 0, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
+            case 16: seqprof_kernel<16><<<grid, 128, 0, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
+            default: seqprof_kernel<32><<<grid, 128, 0, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
+        }
+        g0 = g1;
+    }
+    if (path_dev)
+        seqprof_trace_kernel<<<(unsigned)((n_align + 127) / 128), 128, 0, st>>>(d_desc, (int)n_align, final_state, ws, path_dev, path_len_dev);
+    FAMSA_CUDA(cudaGetLastError());
+    FAMSA_CUDA(cudaFreeAsync(d_desc, st));
+    if (own_state) FAMSA_CUDA(cudaFreeAsync(own_state, st));
+    return FAMSA_OK;
+}

@@ -167,12 +167,13 @@ __device__ __forceinline__ void sweep_block(uint32_t (&V)[W], const uint4* __res
 // per step).  Called by ALL lanes of the warp (`valid` says which lanes own an entry) so that the optional
 // checksum and the guide tree's candidates can use warp reductions.  Returns the entry as a candidate of
 // column j (0 when candidates are off).
+template <bool CAND>
 __device__ __forceinline__ unsigned long long store_pair(const SweepArgs& a, bool valid, uint32_t i, uint32_t j, uint32_t la, uint32_t lb, uint32_t lcs) {
     const int64_t pos = (int64_t)i * (i - 1) / 2 - a.out_base + j;
     uint32_t sim_bits = 0;
     if (valid) {
         if (a.lcs_out) a.lcs_out[pos] = (unsigned short)lcs;
-        if (a.sim_out || a.cand_row) {
+        if (a.sim_out || CAND) {
             const unsigned long long indel = (unsigned long long)la + lb - 2ull * lcs;
             const float sim = __fdiv_rn(__uint2float_rn(lcs), __ull2float_rn(indel * indel));
             if (a.sim_out) a.sim_out[pos] = sim;
@@ -188,7 +189,7 @@ __device__ __forceinline__ unsigned long long store_pair(const SweepArgs& a, boo
             if (a.sim_out && (s_lo | s_hi)) atomicAdd(a.checksum + 1, ((unsigned long long)s_hi << 16) + s_lo);
         }
     }
-    if (a.cand_row) {                                       // kernel-uniform: the guide tree's round-0 candidates
+    if (CAND) {                                             // compile-time: the guide tree's round-0 candidates
         const uint32_t hi = valid ? sim_bits + 1u : 0u;     // similarities are >= +0: bit order == value order
         const uint32_t hmax = __reduce_max_sync(0xffffffffu, hi);
         const uint32_t lmax = __reduce_max_sync(0xffffffffu, hi == hmax ? ~j : 0u);    // ties: the smallest column
@@ -271,7 +272,7 @@ __device__ __forceinline__ void sweep_rows_block(uint32_t (&V)[NR][W], const uin
 // (Without the launch attribute the instruction is a no-op.)
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
-template <int W, int NR>
+template <int W, int NR, bool CAND>
 __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
     extern __shared__ __align__(256) uint8_t smem[];
     asm volatile("griddepcontrol.launch_dependents;");
@@ -316,14 +317,14 @@ __global__ void __launch_bounds__(TB) sweep_short_kernel(const SweepArgs a) {
             for (int w = 0; w < W; ++w) lcs += __popc(~V[p][w]);
             const uint32_t row = i + p;                  // warp-uniform
             if (p == 0) pdl_wait();                      // stores only after the previous launch is complete
-            if (row < r_hi) ckey = max(ckey, store_pair(a, j < row, row, j, a.len[row], lb, lcs));
+            if (row < r_hi) ckey = max(ckey, store_pair<CAND>(a, j < row, row, j, a.len[row], lb, lcs));
         }
-        if (a.cand_col) store_col_cand(a, j, ckey);
+        if (CAND) store_col_cand(a, j, ckey);
     }
 }
 
 // ---- blocked path: rows of nblk blocks x W words; one row per CTA; carry bit-vector per thread --
-template <int W, int CW>
+template <int W, int CW, bool CAND>
 __global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
     extern __shared__ __align__(256) uint8_t smem[];
     asm volatile("griddepcontrol.launch_dependents;");
@@ -361,8 +362,8 @@ __global__ void __launch_bounds__(TB) sweep_long_kernel(const SweepArgs a) {
     }
     if (active) {
         pdl_wait();
-        const unsigned long long ckey = store_pair(a, j < i, i, j, a.len[i], j < i ? a.len[j] : 0, lcs);
-        if (a.cand_col) store_col_cand(a, j, ckey);
+        const unsigned long long ckey = store_pair<CAND>(a, j < i, i, j, a.len[i], j < i ? a.len[j] : 0, lcs);
+        if (CAND) store_col_cand(a, j, ckey);
     }
 }
 
@@ -384,9 +385,13 @@ static cudaError_t launch_sweep(K kernel, const SweepArgs& a, unsigned grid, uns
     return cudaLaunchKernelEx(&cfg, kernel, a);
 }
 
-#define SHORT_CASE(W) case W: return small ? launch_sweep(sweep_short_kernel<W, 1>, a, grid, block, smem, st) \
-                                           : launch_sweep(sweep_short_kernel<W, rows_per_thread(W)>, a, grid, block, smem, st);
-static cudaError_t dispatch_short(int w, bool small, const SweepArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t st) {
+// Variants: small jobs use NR = 1 (one-warp CTAs); the guide tree's sweeps (cand) carry the candidate epilogue
+// as a compile-time variant, so the plain sweep pays nothing for it (measured r02: as a run-time branch it
+// cost the plain sweep 0.8 %).
+#define SHORT_CASE(W) case W: return cand ? launch_sweep(sweep_short_kernel<W, rows_per_thread(W), true>, a, grid, block, smem, st) \
+                                   : small ? launch_sweep(sweep_short_kernel<W, 1, false>, a, grid, block, smem, st) \
+                                           : launch_sweep(sweep_short_kernel<W, rows_per_thread(W), false>, a, grid, block, smem, st);
+static cudaError_t dispatch_short(int w, bool small, bool cand, const SweepArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t st) {
     switch (w) {
         SHORT_CASE(1) SHORT_CASE(2) SHORT_CASE(3) SHORT_CASE(4) SHORT_CASE(5) SHORT_CASE(6) SHORT_CASE(7) SHORT_CASE(8)
         SHORT_CASE(9) SHORT_CASE(10) SHORT_CASE(11) SHORT_CASE(12) SHORT_CASE(13) SHORT_CASE(14) SHORT_CASE(15) SHORT_CASE(16)
@@ -395,9 +400,14 @@ static cudaError_t dispatch_short(int w, bool small, const SweepArgs& a, unsigne
         default: return cudaErrorInvalidValue;
     }
 }
-#define LONG_CASE(W) case W: return launch_sweep(sweep_long_kernel<W, CW_SMALL>, a, grid, TB, smem, st);
-static cudaError_t dispatch_long(int w, bool large, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st) {
-    if (large) return w == 32 ? launch_sweep(sweep_long_kernel<32, CW_LARGE>, a, grid, TB, smem, st) : cudaErrorInvalidValue;
+#define LONG_CASE(W) case W: return cand ? launch_sweep(sweep_long_kernel<W, CW_SMALL, true>, a, grid, TB, smem, st) \
+                                         : launch_sweep(sweep_long_kernel<W, CW_SMALL, false>, a, grid, TB, smem, st);
+static cudaError_t dispatch_long(int w, bool large, bool cand, const SweepArgs& a, unsigned grid, size_t smem, cudaStream_t st) {
+    if (large) {
+        if (w != 32) return cudaErrorInvalidValue;
+        return cand ? launch_sweep(sweep_long_kernel<32, CW_LARGE, true>, a, grid, TB, smem, st)
+                    : launch_sweep(sweep_long_kernel<32, CW_LARGE, false>, a, grid, TB, smem, st);
+    }
     switch (w) {
         LONG_CASE(17) LONG_CASE(18) LONG_CASE(19) LONG_CASE(20) LONG_CASE(21) LONG_CASE(22) LONG_CASE(23) LONG_CASE(24)
         LONG_CASE(25) LONG_CASE(26) LONG_CASE(27) LONG_CASE(28) LONG_CASE(29) LONG_CASE(30) LONG_CASE(31) LONG_CASE(32)
@@ -432,7 +442,8 @@ int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim
     // Then every pair gets its own thread (NR = 1, one row per CTA) in one-warp CTAs, so the hardware
     // scheduler balances the job over the SMs at warp granularity (configs[0]: 124 750 pairs = 3 898 warps
     // over 592 sub-partitions) instead of a few fat 128-thread CTAs per SM.
-    const bool small = small_mode == 1 || (small_mode < 0 && famsa_rows_pairs(i0, i1) < (int64_t)2048 * ctx->sm_count);
+    const bool use_cand = cand != nullptr;
+    const bool small = !use_cand && (small_mode == 1 || (small_mode < 0 && famsa_rows_pairs(i0, i1) < (int64_t)2048 * ctx->sm_count));
     const unsigned block = small ? 32 : TB;
     for (const Bucket& b : ctx->buckets) {
         int64_t lo = std::max(b.r0, std::max<int64_t>(i0, 1)), hi = std::min(b.r1, i1);   // row 0 is empty
@@ -448,13 +459,13 @@ int sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim
                 while (a.ta > nr && (size_t)(a.ta + nr - 1) * wst * ROW_BYTES + 16 > 48 * 1024) a.ta -= nr;   // default dynamic smem limit
                 a.row_tiles = (a.r1 - a.r0 + a.ta - 1) / a.ta;
                 a.cg_tiles = column_group_tiles(ctx, a.r1, a.n_col_tiles, l2_group_bytes);
-                e = dispatch_short(b.wb, small, a, a.row_tiles * a.n_col_tiles, block, (size_t)(a.ta + nr - 1) * wst * ROW_BYTES + 16, st);
+                e = dispatch_short(b.wb, small, use_cand, a, a.row_tiles * a.n_col_tiles, block, (size_t)(a.ta + nr - 1) * wst * ROW_BYTES + 16, st);
             } else {
                 a.n_col_tiles = (a.r1 - 1 + TB - 1) / TB;
                 a.ta = 1;
                 a.row_tiles = a.r1 - a.r0;
                 a.cg_tiles = column_group_tiles(ctx, a.r1, a.n_col_tiles, l2_group_bytes);
-                e = dispatch_long(b.wb, ctx->large_cw, a, a.row_tiles * a.n_col_tiles, (size_t)wst * ROW_BYTES + 16, st);
+                e = dispatch_long(b.wb, ctx->large_cw, use_cand, a, a.row_tiles * a.n_col_tiles, (size_t)wst * ROW_BYTES + 16, st);
             }
             if (e != cudaSuccess) return cuda_fail(e, "sweep kernel launch");
             ctx->launches++;

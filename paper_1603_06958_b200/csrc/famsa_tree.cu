@@ -589,7 +589,8 @@ __global__ void __launch_bounds__(DG_B) tree_dendrogram_kernel(uint32_t k, const
     __shared__ __align__(4) uint16_t s_canon[2 * DG_B + 2];   // smallest slot with the same root (+2: read-ahead slack)
     __shared__ uint16_t s_par[2 * DG_B];                   // local union-find over canonical slots
     __shared__ uint16_t s_hidx[2 * DG_B];
-    __shared__ unsigned long long s_info[2 * DG_B];        // (cluster id << 32 | size) of a local root
+    __shared__ uint2 s_info[2 * DG_B];                     // (.x = size, .y = cluster id) of a local root
+    __shared__ uint32_t s_oa[DG_B], s_ob[DG_B], s_os[DG_B];
     __shared__ uint32_t h_key[DG_H], h_slot[DG_H];
     const uint32_t tid = threadIdx.x, m = k - 1;
     uint32_t nx = 0, ny = 0; float nw = 0.0f;              // this thread's edge of the next batch
@@ -628,31 +629,34 @@ __global__ void __launch_bounds__(DG_B) tree_dendrogram_kernel(uint32_t k, const
         for (uint32_t s = tid; s < 2 * nb; s += DG_B) {
             const uint32_t c = h_slot[s_hidx[s]];
             s_canon[s] = (uint16_t)c;
-            if (c == s) s_info[s] = __ldcg(info + s_root[s]);
+            if (c == s) { const unsigned long long v = __ldcg(info + s_root[s]); s_info[s] = make_uint2((uint32_t)v, (uint32_t)(v >> 32)); }
         }
         __syncthreads();
-        // C: the unions, in edge order
+        // C: the unions, in edge order.  One thread, so what counts is the length of its dependent instruction
+        // chain per edge: 32-bit (id, size) halves, results to shared memory (phase D writes them out, widened).
         if (tid == 0) {
             const uint32_t* canon2 = reinterpret_cast<const uint32_t*>(s_canon);
             uint32_t cc = canon2[0];
+            const uint32_t id0 = k + t0;
             for (uint32_t q = 0; q < nb; ++q) {
                 const uint32_t cnext = canon2[q + 1];      // read ahead (slack entry past the batch)
-                uint32_t x = cc & 0xFFFFu, y = cc >> 16;
+                const uint32_t sx = cc & 0xFFFFu, sy = cc >> 16;
+                uint32_t x = sx, y = sy;
                 uint32_t px = s_par[x], py = s_par[y];
-                unsigned long long ix = s_info[x], iy = s_info[y];   // valid if x, y are local roots (the common case)
-                if (px != x) { do { x = px; px = s_par[x]; } while (px != x); ix = s_info[x]; }
-                if (py != y) { do { y = py; py = s_par[y]; } while (py != y); iy = s_info[y]; }
-                const long long ia = (long long)(ix >> 32), ib = (long long)(iy >> 32);
-                const unsigned long long sz = (ix & 0xFFFFFFFFull) + (iy & 0xFFFFFFFFull);
-                out_a[t0 + q] = ia < ib ? ia : ib; out_b[t0 + q] = ia < ib ? ib : ia; out_size[t0 + q] = (long long)sz;
-                if ((uint32_t)ix < (uint32_t)iy) { const uint32_t s = x; x = y; y = s; }     // the larger set stays the root
-                s_par[y] = (uint16_t)x;
-                s_par[cc & 0xFFFFu] = (uint16_t)x; s_par[cc >> 16] = (uint16_t)x;            // compress both starting slots
-                s_info[x] = ((unsigned long long)(k + t0 + q) << 32) | sz;
+                uint2 ix = s_info[x], iy = s_info[y];      // valid if x, y are local roots (the common case); .x = size, .y = id
+                if (px != x) { do { x = px; px = s_par[x]; } while (px != x); ix = s_info[x]; s_par[sx] = (uint16_t)x; }
+                if (py != y) { do { y = py; py = s_par[y]; } while (py != y); iy = s_info[y]; s_par[sy] = (uint16_t)y; }
+                const uint32_t sz = ix.x + iy.x;
+                s_oa[q] = min(ix.y, iy.y); s_ob[q] = max(ix.y, iy.y); s_os[q] = sz;
+                const bool keep_x = ix.x >= iy.x;            // the larger set stays the root
+                const uint32_t root = keep_x ? x : y, child = keep_x ? y : x;
+                s_par[child] = (uint16_t)root;
+                s_info[root] = make_uint2(sz, id0 + q);
                 cc = cnext;
             }
         }
         __syncthreads();
+        if (tid < nb) { out_a[t0 + tid] = s_oa[tid]; out_b[t0 + tid] = s_ob[tid]; out_size[t0 + tid] = s_os[tid]; }
         // D: back to the global union-find
         for (uint32_t s = tid; s < 2 * nb; s += DG_B) {
             uint32_t f = s_canon[s];
@@ -660,7 +664,7 @@ __global__ void __launch_bounds__(DG_B) tree_dendrogram_kernel(uint32_t k, const
             const uint32_t rf = s_root[f];
             if (s_canon[s] == s) {
                 uf[s_root[s]] = rf;
-                if (f == s) info[rf] = s_info[s];
+                if (f == s) info[rf] = ((unsigned long long)s_info[s].y << 32) | s_info[s].x;
             }
             uf[s_vert[s]] = rf;                            // full compression of the queried leaves
         }

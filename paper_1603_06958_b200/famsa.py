@@ -23,6 +23,8 @@ EXPORTS = ["famsa_pack", "famsa_lcs_rows", "famsa_lcs_rows_host", "famsa_lcs_row
            "famsa_tree_create", "famsa_tree_update", "famsa_tree_merge_edges", "famsa_tree_edge_count",
            "famsa_tree_edges", "famsa_tree_finish", "famsa_tree_free",
            "famsa_guide_tree", "famsa_guide_forest"]
+# include/famsa_profile.h
+EXPORTS_PROFILE = ["famsa_profile_costs", "famsa_gap_scale", "famsa_seqprof_workspace", "famsa_seqprof_align"]
 
 
 class FamsaError(RuntimeError):
@@ -107,6 +109,14 @@ def lib():
         L.famsa_guide_forest.argtypes = [vp, i64, i64, i64, ctypes.POINTER(vp)]
         L.famsa_guide_tree.restype = i32
         L.famsa_guide_tree.argtypes = [vp, i64, vp, vp, vp, vp]
+        L.famsa_profile_costs.restype = i32
+        L.famsa_profile_costs.argtypes = [vp, vp, i64, vp, vp]
+        L.famsa_gap_scale.restype = ctypes.c_double
+        L.famsa_gap_scale.argtypes = [ctypes.c_double] * 3
+        L.famsa_seqprof_workspace.restype = i64
+        L.famsa_seqprof_workspace.argtypes = [vp, vp, i64]
+        L.famsa_seqprof_align.restype = i32
+        L.famsa_seqprof_align.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp]
         L.famsa_strerror.restype = ctypes.c_char_p
         L.famsa_strerror.argtypes = [i32]
         L.famsa_last_error.restype = ctypes.c_char_p
@@ -404,3 +414,45 @@ def famsa_guide_forest(ctx, block_rows=0, part=0, parts=1):
     _check(lib().famsa_guide_forest(ctx.handle, int(block_rows), int(part), int(parts), ctypes.byref(out)))
     t = Tree(out.value, famsa_k(ctx))
     return t
+
+
+# ---- stage III specialisation: sequence-versus-profile DP (include/famsa_profile.h) ----------------
+def famsa_profile_costs(counts, subst, cost, cuda_stream=None):
+    """counts: uint32/int32 CUDA tensor [n][32]; subst: float32 CUDA [32][32]; cost: float32 CUDA [n][32] (output)."""
+    n = counts.shape[0]
+    assert counts.is_cuda and counts.is_contiguous() and counts.element_size() == 4 and counts.shape[1] == 32
+    assert subst.is_cuda and subst.is_contiguous() and subst.element_size() == 4 and subst.numel() == 1024
+    assert cost.is_cuda and cost.is_contiguous() and cost.element_size() == 4 and cost.numel() >= n * 32
+    _check(lib().famsa_profile_costs(_ptr(counts), _ptr(subst), int(n), _ptr(cost), _stream(cuda_stream)))
+
+
+def famsa_gap_scale(k, g_l=45.0, g_d=7.0):
+    return float(lib().famsa_gap_scale(float(k), float(g_l), float(g_d)))
+
+
+def famsa_seqprof_workspace(col_off, seq_off):
+    col_off = np.ascontiguousarray(col_off, dtype=np.int64)
+    seq_off = np.ascontiguousarray(seq_off, dtype=np.int64)
+    assert col_off.size == seq_off.size >= 1
+    n = int(lib().famsa_seqprof_workspace(col_off.ctypes.data, seq_off.ctypes.data, col_off.size - 1))
+    if n < 0:
+        _check(FAMSA_ELENGTH if "residues" in lib().famsa_last_error().decode() else FAMSA_EINVAL)
+    return n
+
+
+def famsa_seqprof_align(cost, col_off, seq, seq_off, gaps, nseq, score, path=None, path_len=None, workspace=None, cuda_stream=None):
+    """cost float32 CUDA [sum n1][32]; col_off / seq_off HOST int64 [B+1]; seq uint8 CUDA; gaps float32 CUDA [B][4];
+    nseq int32 CUDA [B]; score float32 CUDA [B] (output); path uint8 CUDA [sum (n1+n2)] / path_len int32 CUDA [B] /
+    workspace uint8 CUDA [famsa_seqprof_workspace] for the traceback (all three or none)."""
+    col_off = np.ascontiguousarray(col_off, dtype=np.int64)
+    seq_off = np.ascontiguousarray(seq_off, dtype=np.int64)
+    B = col_off.size - 1
+    assert seq_off.size == B + 1
+    for t, size in ((cost, 4), (seq, 1), (gaps, 4), (nseq, 4), (score, 4), (path, 1), (path_len, 4), (workspace, 1)):
+        assert t is None or (t.is_cuda and t.is_contiguous() and t.element_size() == size)
+    assert gaps.numel() >= 4 * B and nseq.numel() >= B and score.numel() >= B
+    if path is not None:
+        assert path.numel() >= int(col_off[-1] + seq_off[-1]) and path_len.numel() >= B
+        assert workspace.numel() >= famsa_seqprof_workspace(col_off, seq_off)
+    _check(lib().famsa_seqprof_align(_ptr(cost), col_off.ctypes.data, _ptr(seq), seq_off.ctypes.data, _ptr(gaps), _ptr(nseq), B,
+                                     _ptr(score), _ptr(path), _ptr(path_len), _ptr(workspace), _stream(cuda_stream)))

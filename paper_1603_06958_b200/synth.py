@@ -246,3 +246,47 @@ def sample_pairs(k, n, seed, lengths_sorted=None, block_rows=1024):
     i = np.concatenate(extra_i); j = np.concatenate(extra_j)
     key = np.unique(i * k + j)
     return key // k, key % k
+
+
+# ---- inputs of the sequence-versus-profile DP ---------------------------------
+def substitution_matrix(seed=SEED_BASE + 40):
+    """A seeded 32 x 32 float32 stand-in for the paper's MIQS matrix (its values are not in
+    the paper): symmetric, diagonal 4..9 in quarter steps, off-diagonal -4..2, symbols >= 25 score -1
+    against everything.  Only its shape and magnitudes matter here."""
+    rng = np.random.default_rng(seed)
+    a = rng.integers(-16, 9, (32, 32)).astype(np.float32) / 4.0
+    s = np.minimum(a, a.T)
+    s[np.arange(32), np.arange(32)] = rng.integers(16, 37, 32).astype(np.float32) / 4.0
+    s[25:, :] = -1.0
+    s[:, 25:] = -1.0
+    return np.ascontiguousarray(s, dtype=np.float32)
+
+
+def profile_batch(n_align, seed, n1_range=(30, 700), nseq_max=40, lengths=None):
+    """n_align independent (profile, sequence) inputs: per alignment an ancestor of n1 residues, a profile of
+    nseq members that differ from it by substitutions (and 5 % gap cells), and one more member with
+    substitutions AND indels as the sequence (<= 1024 residues).
+    `lengths`: optional list of (n1, n2) to force (n2 by cutting / padding the sequence).
+    Returns counts uint32 [sum n1][32], col_off int64, seq uint8, seq_off int64, nseq int32, k_total int."""
+    rng = np.random.default_rng(seed)
+    counts, seqs, col_off, seq_off, nseq = [], [], [0], [0], []
+    for b in range(n_align):
+        n1 = int(lengths[b][0]) if lengths is not None else int(rng.integers(n1_range[0], n1_range[1] + 1))
+        ns = int(rng.integers(1, nseq_max + 1))
+        anc = _draw_bg(rng, n1)
+        d = float(rng.uniform(0.1, 0.4))
+        c = np.zeros((n1, 32), np.uint32)
+        for _ in range(ns):                              # profile members: substitutions only, so columns are aligned;
+            m = anc.copy()                               # 5 % of the cells are gaps (no symbol counted)
+            sub = rng.random(n1) < d
+            m[sub] = _draw_bg(rng, int(sub.sum()))
+            keep = np.flatnonzero(rng.random(n1) >= 0.05)
+            np.add.at(c, (keep, m[keep]), 1)
+        flat, lens = _mutate_batch(rng, anc, np.array([d]))   # the sequence: substitutions and indels
+        y = flat
+        n2 = int(lengths[b][1]) if lengths is not None else int(min(max(y.size, 1), 1024))
+        y = np.concatenate([y, _draw_bg(rng, max(0, n2 - y.size))])[:n2]
+        counts.append(c); seqs.append(y.astype(np.uint8)); nseq.append(ns)
+        col_off.append(col_off[-1] + n1); seq_off.append(seq_off[-1] + n2)
+    return (np.concatenate(counts), np.array(col_off, np.int64), np.concatenate(seqs), np.array(seq_off, np.int64),
+            np.array(nseq, np.int32))

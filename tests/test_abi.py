@@ -28,6 +28,22 @@ def test_exports_match_header(F):
         assert hasattr(L, name), name
 
 
+def test_profile_exports_match_header(F):
+    text = open(os.path.join(ROOT, "include", "famsa_profile.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(famsa_[a-z_]+)\s*\(", text)))
+    assert declared == sorted(F.EXPORTS_PROFILE)
+    L = F.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    # host logic of the NEXT-4 boundary (no GPU needed)
+    assert F.famsa_gap_scale(45) == 1.0
+    assert F.famsa_seqprof_workspace([0, 10, 30], [0, 100, 400]) == 10 * 32 * 4 + 20 * 32 * 16 + 2
+    with pytest.raises(F.FamsaError) as e:
+        F.famsa_seqprof_workspace([0, 10], [0, 2000])         # more than 1024 residues
+    assert e.value.code == F.FAMSA_ELENGTH
+
+
 def test_rows_pairs(F):
     assert F.famsa_rows_pairs(0, 0) == 0
     assert F.famsa_rows_pairs(0, 1) == 0            # row 0 is empty
