@@ -33,7 +33,7 @@ UNIT = "GCUPS"
 BLOCK_ROWS = 1024
 # DRAM traffic of ONE configs[4] step (all its sweep launches), dram__bytes_read.sum + dram__bytes_write.sum per launch
 # from ncu, summed: profiles/r02_ncu_step_traffic.md.  Not measurable outside a profiler, so a recorded figure.
-NCU_STEP_TRAFFIC = {"config": 4, "bytes": None, "launches": None, "source": "profiles/r02_ncu_step_traffic.md"}
+NCU_STEP_TRAFFIC = {"config": 4, "bytes": 3.546273e+10, "launches": 39, "source": "profiles/r02_ncu_step_traffic.md"}
 ALU_INSTR_PER_CELL = 3.0 / 32.0      # LOP3 + IADD3.X + LOP3 per 32-bit word-step
 WORKLOADS = {
     0: "configs[0]: k=500, one family, all 124750 pairs",
@@ -63,6 +63,9 @@ def parse_args():
     ap.add_argument("--no-guide-tree", action="store_true", help="skip the stages I+II leg that N=1 runs by default")
     ap.add_argument("--tune", default=None, help="rows_per_cta,small_job_mode,l2_group_mb for famsa_ctx_set_tuning (experiments)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU work per oracle sample")
+    ap.add_argument("--workload", default="lcs", choices=["lcs", "seqprof"],
+                    help="lcs: the all-pairs LCS sweep (the headline, default); seqprof: SURVEY 8(f) NEXT-4, a batch of sequence-vs-profile alignments")
+    ap.add_argument("--batch", type=int, default=8192, help="alignments per step of --workload seqprof")
     ap.add_argument("--kernel-only", action="store_true",
                     help="profiling runs: only the device-resident timed steps (no e2e, full-sweep, guide-tree or CPU legs)")
     ap.add_argument("--host-mode", type=int, default=-1, choices=[-1, 0, 1],
@@ -366,17 +369,26 @@ def run_cuda(args, rank, world, local_rank):
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
+    # Per-step events only when a step is long: an event record between two sweep launches is a stream operation
+    # that is not a kernel, so the next launch cannot start programmatically while its predecessor drains (6.5),
+    # and a 0.1 ms step (configs[0]) would be measured without the overlap that back-to-back calls really get.
+    probe = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    probe[0].record(stream); step(); probe[1].record(stream); torch.cuda.synchronize()
+    per_step_events = probe[0].elapsed_time(probe[1]) > 5.0
+    ck.zero_()
+    barrier()
     l0 = F.famsa_launch_count(ctx)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     ev[0].record(stream)
     for s in range(args.steps):
         step()
-        ev[s + 1].record(stream)
+        if per_step_events or s == args.steps - 1:
+            ev[s + 1].record(stream)
     barrier()
     clocks = sampler.stop()
     launches = F.famsa_launch_count(ctx) - l0
     ms_total = ev[0].elapsed_time(ev[-1])
-    step_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)]
+    step_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)] if per_step_events else None
     ms_rank = ms_total
     ms_total, cells_all, pairs_all = reduce_over_ranks(dist, ms_total, cells_step, pairs_step, dev)
     sec = ms_total * 1e-3
@@ -638,8 +650,102 @@ def run_cuda(args, rank, world, local_rank):
         sys.exit(3)
 
 
+def run_seqprof(args, rank, world, local_rank):
+    """one step = one batch of independent sequence-vs-profile alignments (profile costs from
+    the counters, DP with traceback), inputs resident in HBM; e2e = the same through the C ABI from pinned host
+    arrays with the scores, paths and path lengths read back.  Metric: DP cells (n1 x n2) per second."""
+    import torch
+    from paper_1603_06958_b200 import famsa as F, synth
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    B = args.batch
+    counts, col_off, seq, seq_off, nseq = synth.profile_batch(B, seed=SEQPROF_SEED + rank, n1_range=(100, 700))
+    subst = synth.substitution_matrix()
+    gaps = np.tile(np.array([0.66, 0.66, 14.85, 1.25], np.float32) * np.float32(F.famsa_gap_scale(B)), (B, 1))
+    n1 = np.diff(col_off); n2 = np.diff(seq_off)
+    cells = float((n1 * n2).sum())
+    h = {"counts": torch.from_numpy(counts.astype(np.int32)).pin_memory(), "seq": torch.from_numpy(seq).pin_memory(),
+         "gaps": torch.from_numpy(gaps).pin_memory(), "nseq": torch.from_numpy(nseq).pin_memory(), "subst": torch.from_numpy(subst).pin_memory()}
+    d = {k_: v.to(dev) for k_, v in h.items()}
+    cost = torch.empty((counts.shape[0], 32), dtype=torch.float32, device=dev)
+    score = torch.empty(B, dtype=torch.float32, device=dev)
+    path = torch.empty(int(col_off[-1] + seq_off[-1]), dtype=torch.uint8, device=dev)
+    plen = torch.empty(B, dtype=torch.int32, device=dev)
+    ws = torch.empty(F.famsa_seqprof_workspace(col_off, seq_off), dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step(src):
+        F.famsa_profile_costs(src["counts"], src["subst"], cost, stream)
+        F.famsa_seqprof_align(cost, col_off, src["seq"], seq_off, src["gaps"], src["nseq"], score, path, plen, ws, stream)
+    for _ in range(args.warmup):
+        step(d)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank); sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step(d)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    value = cells * args.steps / ms / 1e6
+    # e2e: pinned host inputs -> device, results back to pinned host, every step
+    h_score = torch.empty(B, dtype=torch.float32).pin_memory(); h_path = torch.empty(path.numel(), dtype=torch.uint8).pin_memory()
+    h_plen = torch.empty(B, dtype=torch.int32).pin_memory()
+    def e2e_step():
+        src = {k_: v.to(dev, non_blocking=True) for k_, v in h.items()}
+        step(src)
+        h_score.copy_(score, non_blocking=True); h_path.copy_(path, non_blocking=True); h_plen.copy_(plen, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        e2e_step()
+    e2e_sec = time.perf_counter() - t0
+    # the oracle beside it and against it: a bounded sample of the batch (fp32 mode: same-precision decisions)
+    cpu = parity = None
+    if not args.no_cpu and rank == 0:
+        from oracle import profile_oracle as po
+        hc = cost.cpu().numpy(); hs = score.cpu().numpy(); hp = path.cpu().numpy(); hl = plen.cpu().numpy()
+        rng = np.random.default_rng(5); pick = rng.permutation(B)[:min(B, 4000)]
+        t0 = time.perf_counter(); bad = 0; ccells = 0.0
+        for b in pick:
+            s32, p32 = po.align(hc[col_off[b]:col_off[b + 1]], seq[seq_off[b]:seq_off[b + 1]], gaps[b], int(nseq[b]), want_path=True, precision="f32")
+            end = int(col_off[b + 1] + seq_off[b + 1])
+            bad += int(not (hs[b] == np.float32(s32) and np.array_equal(hp[end - hl[b]:end], p32)))
+            ccells += float(n1[b] * n2[b])
+            if time.perf_counter() - t0 > args.cpu_seconds:
+                break
+        dt = time.perf_counter() - t0
+        cpu = {"value": ccells / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": "oracle/profile_oracle.c (fp32 mode, with traceback) on seeded alignments of the batch for %.1f s, one thread" % dt}
+        parity = {"alignments": int(ccells > 0) and int(np.searchsorted(np.cumsum(n1[pick] * n2[pick]), ccells) + 1), "mismatch": bad,
+                  "what": "score bit-exact and path identical to the oracle's fp32 mode"}
+    line = {"metric": "seqprof_dp_gcups", "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "SURVEY 8(f) NEXT-4: %d independent sequence-vs-profile alignments per step (profiles of 100-700 columns from 1-40 "
+                                   "sequences, sequences with indels), costs + DP + traceback" % B,
+                       "cells_per_step": cells, "l2": "direction matrices (%.2f GB per step) exceed L2" % (ws.numel() / 1e9)},
+            "alignments_per_s": B * args.steps / ms * 1e3,
+            "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"], "samples": clocks["samples"]},
+            "e2e": {"value": cells * args.steps / e2e_sec / 1e9, "unit": UNIT,
+                    "h2d_bytes_per_step": int(sum(v.numel() * v.element_size() for v in h.values())),
+                    "d2h_bytes_per_step": int(h_score.numel() * 4 + h_path.numel() + h_plen.numel() * 4)},
+            "gpu_launches": 6 * args.steps, "cpu_baseline": cpu, "parity_in_bench": parity}
+    print(json.dumps(line), flush=True)
+    if parity is not None and parity["mismatch"]:
+        sys.exit(3)
+
+
+SEQPROF_SEED = 160306958 + 50
+
+
 def main():
     args = parse_args()
+    if args.workload == "seqprof":
+        run_seqprof(args, int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0")))
+        return
     if args.kernel_only:
         args.no_cpu = args.no_full = args.no_guide_tree = True
     rank = int(os.environ.get("RANK", "0"))

@@ -3,7 +3,7 @@
 // DESIGN.md P1-P9.
 //
 // Mapping: one warp per alignment.  The SEQUENCE side (n2 <= 1024 residues) is spread over the 32 lanes, J =
-// 4 / 8 / 16 / 32 consecutive residues per lane, and for each of them the lane keeps the three states of the
+// 4, 8, ... 32 consecutive residues per lane, and for each of them the lane keeps the three states of the
 // previous profile column (row) in registers: 3 J floats.  The rows are swept in a skewed wavefront: at step t
 // lane l computes row t - l + 1, so what it needs from the left -- the three states of lane l-1's last residue
 // in the same row -- was produced one step earlier and arrives by one __shfl_up per state; the value received
@@ -146,7 +146,8 @@ __global__ void seqprof_trace_kernel(const AlignDesc* __restrict__ desc, int n, 
     path_len[d.idx] = len;
 }
 
-static int lanes_j(int64_t n2) { return n2 <= 128 ? 4 : (n2 <= 256 ? 8 : (n2 <= 512 ? 16 : 32)); }
+// residues per lane: the smallest multiple of 4 with 32 J >= n2 (4 .. 32), so at most 127 of the 32 J lane slots idle
+static int lanes_j(int64_t n2) { return (int)(4 * ((n2 + 127) / 128)); }
 
 }  // namespace famsa
 
@@ -230,12 +231,12 @@ extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off
         while (g1 < n_align && sorted[(size_t)g1].j == sorted[(size_t)g0].j) ++g1;
         const int n = (int)(g1 - g0);
         const unsigned grid = (unsigned)((n + 3) / 4);       // 4 warps = 4 alignments per CTA
+#define SEQPROF_CASE(JJ) case JJ: seqprof_kernel<JJ><<<grid, 128, 0, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
         switch (sorted[(size_t)g0].j) {
-            case 4:  seqprof_kernel<4><<<grid, 128, 0, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
-            case 8:  seqprof_kernel<8><<<grid, 128, 0, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
-            case 16: seqprof_kernel<16><<<grid, 128, 0, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
+            SEQPROF_CASE(4) SEQPROF_CASE(8) SEQPROF_CASE(12) SEQPROF_CASE(16) SEQPROF_CASE(20) SEQPROF_CASE(24) SEQPROF_CASE(28)
             default: seqprof_kernel<32><<<grid, 128, 0, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
         }
+#undef SEQPROF_CASE
         g0 = g1;
     }
     if (path_dev)
