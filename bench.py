@@ -79,6 +79,19 @@ def step_blocks(k, stride, offset=0):
     return [(b * BLOCK_ROWS, min((b + 1) * BLOCK_ROWS, k)) for b in range(offset % max(stride, 1), nblocks, stride)]
 
 
+def step_config(config, k, stride, blocks, pairs_step, cells_step, want_sim):
+    """The `config` object of the JSON line: the same for the CUDA arm and the reference arm."""
+    out_bytes = pairs_step * (2 + (4 if want_sim else 0))
+    if out_bytes > 126e6:
+        l2_note = "no flush needed: every step writes %.2f GB of row-block output (> 126 MB L2) between re-reads" % (out_bytes / 1e9)
+    else:
+        l2_note = "working set fits L2 (small config); ALU-bound path, no L2 flush between steps"
+    return {"workload": WORKLOADS[config], "k": k,
+            "step": ("all rows" if stride == 1 else "every %d-th %d-row block (%d blocks)" % (stride, BLOCK_ROWS, len(blocks))),
+            "pairs_per_step": pairs_step, "cells_per_step": cells_step, "outputs": "uint16 LCS" + (" + fp32 similarity" if want_sim else ""),
+            "l2": l2_note, "parallelism": "replicated set, row blocks dealt per rank, no collective"}
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -212,6 +225,12 @@ def run_reference(args, rank, world):
     blocks = step_blocks(k, 1 if args.full else stride)
     want_sim = args.config != 3
     secs = min(args.cpu_seconds, 8.0)
+    # the CUDA arm's step, described identically (exact integer sums: every value is below 2^53)
+    from oracle import famsa_oracle
+    lens = np.diff(offsets)[famsa_oracle.sort_perm(offsets)].astype(np.int64)
+    prefix = np.concatenate([[0], np.cumsum(lens)])
+    pairs_cfg = int(sum(b * (b - 1) // 2 - a * (a - 1) // 2 for a, b in blocks))
+    cells_cfg = float(sum(int((lens[a:b] * prefix[a:b]).sum()) for a, b in blocks))
     times, cells_step, pairs_step, cores = [], 0.0, 0, 1
     for s in range(args.warmup + args.steps):
         pi, pj, cells, cores, _, _ = oracle_sample(seqs, offsets, blocks, secs, seed=1000 + s)
@@ -225,7 +244,7 @@ def run_reference(args, rank, world):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total / max(args.steps, 1) * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-        "config": {"workload": WORKLOADS[args.config], "k": k, "step": "bounded oracle sample of the cuda arm's step"},
+        "config": step_config(args.config, k, 1 if args.full else stride, blocks, pairs_cfg, cells_cfg, want_sim),
         "pairs_per_s": pairs_step / total,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -604,19 +623,11 @@ def run_cuda(args, rank, world, local_rank):
         "frac_of_nominal_64_per_clk_sm_at_max_clock": achieved / nominal,
         "roofline_gcups": p_int / ALU_INSTR_PER_CELL / 1e9,
     }
-    if out_bytes > 126e6:
-        l2_note = "no flush needed: every step writes %.2f GB of row-block output (> 126 MB L2) between re-reads" % (out_bytes / 1e9)
-    else:
-        l2_note = "working set fits L2 (small config); ALU-bound path, no L2 flush between steps"
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong" if args.strong else "weak", "vs_baseline": None,
         "dtype": "u32", "data": "synthetic",
-        "config": {"workload": WORKLOADS[args.config], "k": k,
-                   "step": ("all rows" if stride == 1 else "every %d-th %d-row block (%d blocks)" % (stride, BLOCK_ROWS, len(blocks))),
-                   "pairs_per_step": pairs_step, "cells_per_step": cells_step, "outputs": "uint16 LCS" + (" + fp32 similarity" if want_sim else ""),
-                   "l2": l2_note,
-                   "parallelism": "replicated set, row blocks dealt per rank, no collective"},
+        "config": step_config(args.config, k, stride, blocks, pairs_step, cells_step, want_sim),
         "pairs_per_s": pairs_all * args.steps / sec,
         "step_ms": step_ms, "pack_ms": pack_ms,
         "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"], "samples": clocks["samples"]},
