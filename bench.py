@@ -163,17 +163,17 @@ def oracle_sample(seqs, offsets, blocks, cpu_seconds, seed, n=400000):
 def time_bitparallel(seqs, offsets, blocks, seconds, seed):
     """CONTEXT figure: the paper's own CPU design (64-bit bit-parallel LCS, several pairs per SIMD register,
     rows over threads; oracle/bitpar_cpu.c) on a bounded sample of the step: seeded rows of the step's row
-    blocks, 64 seeded columns j < i each (the row's match table is built once, as in the paper's design).
+    blocks, 128 seeded columns j < i each (the row's match table is built once, as in the paper's design).
     Every ISA variant the host runs is timed after a pilot that sizes the sample for ~`seconds` of work."""
     from oracle import famsa_oracle
     cores = famsa_oracle.n_threads_default()
     perm = famsa_oracle.sort_perm(offsets)
     lens = np.diff(offsets)[perm].astype(np.int64)
-    rows_all = np.concatenate([np.arange(max(a, 64), b, dtype=np.int64) for a, b in blocks if b > 64]) if blocks else np.zeros(0, np.int64)
+    rows_all = np.concatenate([np.arange(max(a, 128), b, dtype=np.int64) for a, b in blocks if b > 128]) if blocks else np.zeros(0, np.int64)
     if rows_all.size == 0:
         return None
     rng = np.random.default_rng(seed)
-    ncol = 64
+    ncol = 128
 
     def sample(n_rows):
         ri = rng.choice(rows_all, size=n_rows, p=rows_all / rows_all.sum())
