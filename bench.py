@@ -701,6 +701,15 @@ def run_seqprof(args, rank, world, local_rank):
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1)
     value = cells * args.steps / ms / 1e6
+    peak = F.famsa_alu_peak(local_rank)
+    # Roofline: the ALU pipe.  Per cell and state: 2 compares + 2 value selects + 2 direction selects on
+    # the ALU pipe (18 per cell; the 7 fp32 adds / subtracts run on the FMA pipe beside them).
+    alu_per_cell = 18.0
+    roofline = {"bound": "alu", "achieved": cells * args.steps * alu_per_cell / (ms * 1e-3) / 1e12, "peak": peak["instr_per_s"] / 1e12,
+                "unit": "TIOP/s (ALU-pipe lane-instr)", "frac": cells * args.steps * alu_per_cell / (ms * 1e-3) / peak["instr_per_s"],
+                "traffic": None, "algorithmic_instr_per_cell": alu_per_cell, "kernel": "famsa::seqprof_kernel<J>",
+                "peak_source": "famsa_alu_peak micro-kernel, measured in this run",
+                "note": "padding of n2 to 32 J lane slots, the 31-step skew of the wavefront and the traceback all count against the kernel"}
     # e2e: pinned host inputs -> device, results back to pinned host, every step
     h_score = torch.empty(B, dtype=torch.float32).pin_memory(); h_path = torch.empty(path.numel(), dtype=torch.uint8).pin_memory()
     h_plen = torch.empty(B, dtype=torch.int32).pin_memory()
@@ -743,7 +752,7 @@ def run_seqprof(args, rank, world, local_rank):
             "e2e": {"value": cells * args.steps / e2e_sec / 1e9, "unit": UNIT,
                     "h2d_bytes_per_step": int(sum(v.numel() * v.element_size() for v in h.values())),
                     "d2h_bytes_per_step": int(h_score.numel() * 4 + h_path.numel() + h_plen.numel() * 4)},
-            "gpu_launches": 6 * args.steps, "cpu_baseline": cpu, "parity_in_bench": parity}
+            "gpu_launches": 10 * args.steps, "roofline": roofline, "cpu_baseline": cpu, "parity_in_bench": parity}
     print(json.dumps(line), flush=True)
     if parity is not None and parity["mismatch"]:
         sys.exit(3)

@@ -286,6 +286,62 @@ def test_alu_peak_is_sane(F):
     assert p["instr_per_s"] == pytest.approx(p["instr_per_clk_sm"] * p["sm_mhz"] * 1e6 * 148, rel=0.05)
 
 
+def test_checksum_epilogue_against_the_oracle(F, oracle):
+    """famsa_lcs_rows_checksum ("a 64-bit checksum per block ... to prove the work was done"): the sums
+    the kernels' epilogue accumulates equal the ORACLE's sum of LCS lengths and the sum of the stored fp32 bit patterns,
+    for the register path in both CTA shapes and for the blocked long path; the call ADDS to what is there."""
+    import torch
+    from paper_1603_06958_b200 import synth
+    for cfg, k, seed in ((1, 700, 55), (2, 260, 56)):
+        seqs, offsets = synth.family(cfg, k=k, seed=seed)
+        lref, _ = oracle.rows(seqs, offsets, 0, k)
+        n = F.famsa_rows_pairs(0, k)
+        with F.famsa_pack(seqs, offsets) as ctx:
+            for small in (0, 1):
+                F.famsa_ctx_set_tuning(ctx, 0, small, 0)
+                lcs = torch.zeros(n, dtype=torch.uint16, device="cuda")
+                sim = torch.zeros(n, dtype=torch.float32, device="cuda")
+                ck = torch.tensor([5, 7], dtype=torch.int64, device="cuda")
+                F.famsa_lcs_rows_checksum(ctx, 0, k // 2, lcs, sim, ck)
+                half = F.famsa_rows_pairs(0, k // 2)
+                F.famsa_lcs_rows_checksum(ctx, k // 2, k, lcs[half:], sim[half:], ck)
+                torch.cuda.synchronize()
+                c = ck.cpu().numpy()
+                assert int(c[0]) - 5 == int(lref.sum())
+                bits = int(sim.cpu().numpy().view(np.uint32).astype(np.uint64).sum())
+                assert (int(c[1]) - 7) % 2 ** 64 == bits % 2 ** 64
+                assert np.array_equal(lcs.cpu().numpy().astype(np.int64), lref)
+                ck2 = torch.zeros(2, dtype=torch.int64, device="cuda")
+                F.famsa_lcs_rows_checksum(ctx, 0, k, lcs, None, ck2)       # LCS only: [1] untouched
+                torch.cuda.synchronize()
+                assert ck2.cpu().numpy().tolist() == [int(lref.sum()), 0]
+
+
+def test_profiling_getters(F):
+    """famsa_mix_peak (the instruction-mix ceiling printed in every bench line), the per-phase timers of the host path
+    in both modes, famsa_pack_profile, famsa_trim."""
+    import torch
+    from paper_1603_06958_b200 import synth
+    m = F.famsa_mix_peak(0)
+    assert 45.0 < m["alu_instr_per_clk_sm"] <= F.famsa_alu_peak(0)["instr_per_clk_sm"] + 0.5
+    seqs, offsets = synth.family(1, k=900, seed=57)
+    n = F.famsa_rows_pairs(0, 900)
+    with F.famsa_pack(seqs, offsets) as ctx:
+        pp = F.famsa_pack_profile(ctx)
+        assert all(v >= 0.0 for v in pp.values()) and sum(pp.values()) > 0.0
+        F.famsa_host_profile(ctx, True)
+        hl = torch.empty(n, dtype=torch.uint16).pin_memory(); hs = torch.empty(n, dtype=torch.float32).pin_memory()
+        F.famsa_lcs_rows_host(ctx, 0, 900, hl, hs)                          # pinned: direct stores
+        p = F.famsa_host_profile_read(ctx)
+        assert p["chunks"] == 1 and p["d2h_ms"] == 0.0 and p["sweep_ms"] > 0.0 and p["d2h_bytes"] == 6.0 * n
+        nl = np.empty(n, np.uint16); nsim = np.empty(n, np.float32)
+        F.famsa_lcs_rows_host(ctx, 0, 900, nl, nsim)                        # pageable: staged chunks + copies
+        p = F.famsa_host_profile_read(ctx)
+        assert p["chunks"] >= 1 and p["d2h_ms"] > 0.0 and p["sweep_ms"] > 0.0 and p["d2h_bytes"] == 6.0 * n
+        assert np.array_equal(nl, hl.numpy().view(np.uint16)) and np.array_equal(nsim, hs.numpy())
+    F.famsa_trim()
+
+
 def test_gpu_matches_stored_oracle_digests(F):
     """The CUDA path against digests the oracle wrote earlier (tests/golden/oracle_digests.txt): the
     expected values do not come from this run, nor ever from the CUDA path."""
