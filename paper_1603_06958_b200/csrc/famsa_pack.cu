@@ -170,14 +170,26 @@ extern "C" int famsa_pack(const uint8_t* seqs, const int64_t* offsets, int64_t k
 }
 
 namespace {
-struct DevTmp {                       // frees scratch on every exit path of pack_impl
-    std::vector<void*> ptrs;
-    ~DevTmp() { for (void* p : ptrs) cudaFree(p); }
+struct DevTmp {                       // pack_impl's scratch: ONE device allocation carved up (a cudaMalloc / cudaFree pair
+    uint8_t* base = nullptr;          // per piece cost famsa_pack ~2 ms), freed on every exit path
+    size_t cap = 0, used = 0;
+    std::vector<void*> extra;         // pieces that did not fit the reservation (never with the sizes pack_impl reserves)
+    ~DevTmp() { cudaFree(base); for (void* p : extra) cudaFree(p); }
+    static size_t padded(size_t bytes) { return (std::max<size_t>(bytes, 1) + 255) & ~(size_t)255; }
+    int reserve(size_t bytes) {
+        cudaError_t e = cudaMalloc((void**)&base, std::max<size_t>(bytes, 256));
+        if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); famsa::set_error("famsa_pack: device allocation failed"); return FAMSA_ENOMEM; }
+        if (e != cudaSuccess) return famsa::cuda_fail(e, "cudaMalloc");
+        cap = std::max<size_t>(bytes, 256);
+        return FAMSA_OK;
+    }
     template <typename T> int alloc(T** p, size_t n) {
+        const size_t bytes = padded(n * sizeof(T));
+        if (used + bytes <= cap) { *p = reinterpret_cast<T*>(base + used); used += bytes; return FAMSA_OK; }
         cudaError_t e = famsa::dalloc(p, n);
         if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); famsa::set_error("famsa_pack: device allocation failed"); return FAMSA_ENOMEM; }
         if (e != cudaSuccess) return famsa::cuda_fail(e, "cudaMalloc");
-        ptrs.push_back(*p);
+        extra.push_back(*p);
         return FAMSA_OK;
     }
 };
@@ -199,14 +211,16 @@ static int pack_impl(const uint8_t* seqs, const int64_t* offsets, int64_t k, int
         return FAMSA_ECUDA;
     }
     FAMSA_CUDA(cudaSetDevice(device));
-    cudaDeviceProp prop;
-    FAMSA_CUDA(cudaGetDeviceProperties(&prop, device));
-    if (prop.major != 10) {
-        set_error("famsa_pack: device is sm_" + std::to_string(prop.major * 10 + prop.minor) +
+    int cc_major = 0, cc_minor = 0, sm_count = 0;            // (cudaGetDeviceProperties costs ~1 ms per call: attributes instead)
+    FAMSA_CUDA(cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, device));
+    FAMSA_CUDA(cudaDeviceGetAttribute(&cc_minor, cudaDevAttrComputeCapabilityMinor, device));
+    FAMSA_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, device));
+    if (cc_major != 10) {
+        set_error("famsa_pack: device is sm_" + std::to_string(cc_major * 10 + cc_minor) +
                   ", this library is built for sm_100a only");
         return FAMSA_ECUDA;
     }
-    ctx->device = device; ctx->sm_count = prop.multiProcessorCount; ctx->k = k;
+    ctx->device = device; ctx->sm_count = sm_count; ctx->k = k;
     ctx->n_groups = (k + GROUP - 1) / GROUP;
     const int64_t total = offsets[k];
     using clk = std::chrono::steady_clock;
@@ -214,6 +228,11 @@ static int pack_impl(const uint8_t* seqs, const int64_t* offsets, int64_t k, int
     clk::time_point t_phase = clk::now();
     DevTmp tmp;
     cudaStream_t st = nullptr;           // legacy default stream; pack synchronises before returning
+    size_t cub_bytes = 0;
+    if (k > 0) FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, cub_bytes, (uint32_t*)nullptr, (uint32_t*)nullptr, (uint32_t*)nullptr,
+                                                         (uint32_t*)nullptr, (int)k, 0, 16, st));
+    FAMSA_TRY(tmp.reserve(2 * DevTmp::padded((size_t)total) + DevTmp::padded(8 * ((size_t)k + 1)) + DevTmp::padded(8) +
+                          4 * DevTmp::padded(4 * (size_t)k) + DevTmp::padded(cub_bytes) + DevTmp::padded(12 * (size_t)k)));
 
     // ---- a1 encode
     uint8_t *d_raw = nullptr, *d_codes = nullptr; int64_t* d_off = nullptr; unsigned long long* d_bad = nullptr;
@@ -247,8 +266,6 @@ static int pack_impl(const uint8_t* seqs, const int64_t* offsets, int64_t k, int
     if (k > 0) {
         sortkey_kernel<<<(unsigned)((k + 255) / 256), 256, 0, st>>>(d_off, k, d_key, d_idx);
         ctx->launches++;
-        size_t cub_bytes = 0;
-        FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, cub_bytes, d_key, d_key2, d_idx, d_perm, (int)k, 0, 16, st));
         void* d_cub = nullptr;
         FAMSA_TRY(tmp.alloc((uint8_t**)&d_cub, cub_bytes));
         FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(d_cub, cub_bytes, d_key, d_key2, d_idx, d_perm, (int)k, 0, 16, st));

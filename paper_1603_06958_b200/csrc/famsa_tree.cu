@@ -454,11 +454,10 @@ extern "C" int famsa_tree_create(int64_t k, int device, famsa_tree** out) {
     famsa_tree* t = new (std::nothrow) famsa_tree();
     if (!t) { set_error("famsa_tree_create: host allocation failed"); return FAMSA_ENOMEM; }
     t->device = device; t->k = k;
-    cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); famsa_tree_free(t); set_error("famsa_tree_create: cudaGetDeviceProperties"); return FAMSA_ECUDA; }
-    t->sm_count = prop.multiProcessorCount;
-    int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tree_merge_kernel, 256, 0) != cudaSuccess || per_sm < 1 || !prop.cooperativeLaunch) {
+    int coop = 0, per_sm = 0;
+    if (cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tree_merge_kernel, 256, 0) != cudaSuccess || per_sm < 1 || !coop) {
         cudaGetLastError(); famsa_tree_free(t); set_error("famsa_tree_create: the device cannot run the cooperative merge kernel"); return FAMSA_ECUDA;
     }
     t->merge_grid = t->sm_count;                           // one 256-thread CTA per SM: co-resident beside the sweep's CTAs
