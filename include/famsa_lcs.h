@@ -142,8 +142,10 @@ int famsa_pack_profile(const famsa_ctx* ctx, double* ms4);
 
 /*
  * The HOST-output path keeps its device staging (two row-chunk buffers, two streams) in a process-wide pool:
- * famsa_free returns a ctx's set to the pool and the next ctx on that device reuses it.  famsa_trim()
- * releases every idle set (call it before a large allocation of your own).
+ * famsa_free returns a ctx's set to the pool and the next ctx on that device reuses it.  famsa_free likewise keeps
+ * the ctx's device blocks (the packed set, up to 6 GB per process) for the next famsa_pack of about the same size,
+ * so that pack / sweep / free in a loop does not go through cudaMalloc and cudaFree.  famsa_trim() releases every
+ * idle set and block (call it before a large allocation of your own).
  */
 int famsa_trim(void);
 

@@ -112,6 +112,9 @@ void set_error(const std::string& msg);
 int  cuda_fail(cudaError_t e, const char* what);          // records text, returns FAMSA_ECUDA
 int  sweep_rows(famsa_ctx* ctx, int64_t i0, int64_t i1, uint16_t* lcs, float* sim, unsigned long long* checksum, const TreeCand* cand, cudaStream_t st);
 void staging_release(Staging* s);                          // back to the pool (drains its streams first)
+cudaError_t cache_alloc(int device, void** p, size_t bytes);   // device block cache of famsa_pack / famsa_free (famsa_pack.cu)
+void cache_free(void* p);
+void cache_trim();
 }  // namespace famsa
 
 #define FAMSA_CUDA(call)                                                     \

@@ -119,8 +119,63 @@ __global__ void table_kernel(const uint8_t* __restrict__ codes, const int64_t* _
     }
 }
 
+// ---- device block cache: famsa_pack / famsa_free in a loop (the end-to-end path of a streaming caller) would
+// otherwise pay ~10 cudaMalloc + cudaFree of up to 0.5 GB each per call, whose latency varies between 1 and 50 ms
+// with the state of the process' address space (measured r02).  Freed blocks are kept (up to CACHE_LIMIT bytes per
+// process) and handed to the next allocation of about the same size on the same device; famsa_trim() releases them.
+struct CachedBlock { int device; void* p; size_t bytes; };
+static std::mutex g_cache_mu;
+static std::vector<CachedBlock> g_cache;                 // idle blocks
+static std::vector<CachedBlock> g_live;                  // blocks handed out (to know their size when they come back)
+static size_t g_cache_bytes = 0;
+constexpr size_t CACHE_LIMIT = (size_t)6 << 30;
+
+cudaError_t cache_alloc(int device, void** p, size_t bytes) {
+    bytes = (std::max<size_t>(bytes, 1) + 255) & ~(size_t)255;
+    {
+        std::lock_guard<std::mutex> lk(g_cache_mu);
+        int best = -1;
+        for (size_t n = 0; n < g_cache.size(); ++n) {
+            const CachedBlock& b = g_cache[n];
+            if (b.device == device && b.bytes >= bytes && b.bytes <= bytes + bytes / 8 + 4096 &&
+                (best < 0 || b.bytes < g_cache[best].bytes)) best = (int)n;
+        }
+        if (best >= 0) {
+            *p = g_cache[best].p;
+            g_live.push_back(g_cache[best]); g_cache_bytes -= g_cache[best].bytes;
+            g_cache.erase(g_cache.begin() + best);
+            return cudaSuccess;
+        }
+    }
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); cache_trim(); e = cudaMalloc(p, bytes); }   // the cache must never cause an OOM
+    if (e == cudaSuccess) { std::lock_guard<std::mutex> lk(g_cache_mu); g_live.push_back(CachedBlock{device, *p, bytes}); }
+    return e;
+}
+
+// The caller guarantees that nothing on the device still uses the block (famsa_free synchronises the device first).
+void cache_free(void* p) {
+    if (!p) return;
+    CachedBlock b{-1, nullptr, 0};
+    {
+        std::lock_guard<std::mutex> lk(g_cache_mu);
+        for (size_t n = 0; n < g_live.size(); ++n)
+            if (g_live[n].p == p) { b = g_live[n]; g_live.erase(g_live.begin() + n); break; }
+        if (b.p && g_cache_bytes + b.bytes <= CACHE_LIMIT) { g_cache.push_back(b); g_cache_bytes += b.bytes; return; }
+    }
+    cudaFree(p);
+}
+
+void cache_trim() {
+    std::vector<CachedBlock> all;
+    { std::lock_guard<std::mutex> lk(g_cache_mu); all.swap(g_cache); g_cache_bytes = 0; }
+    int cur = 0; cudaGetDevice(&cur);
+    for (const CachedBlock& b : all) { cudaSetDevice(b.device); cudaFree(b.p); }
+    cudaSetDevice(cur);
+}
+
 template <typename T>
-static cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, std::max<size_t>(n, 1) * sizeof(T)); }
+static cudaError_t dalloc(int device, T** p, size_t n) { return cache_alloc(device, (void**)p, std::max<size_t>(n, 1) * sizeof(T)); }
 
 }  // namespace famsa
 
@@ -132,8 +187,9 @@ extern "C" void famsa_free(famsa_ctx* ctx) {
     if (ctx->stg) famsa::staging_release(ctx->stg);       // drains the host path's streams, then back to the pool
     if (ctx->s_direct) { cudaStreamSynchronize(ctx->s_direct); cudaStreamDestroy(ctx->s_direct); }
     for (famsa::HostChunkTimers& t : ctx->direct_timers) for (cudaEvent_t e : t.ev) if (e) cudaEventDestroy(e);
-    cudaFree(ctx->d_stream); cudaFree(ctx->d_tables); cudaFree(ctx->d_len);
-    cudaFree(ctx->d_toff); cudaFree(ctx->d_goff);
+    cudaDeviceSynchronize();                              // as cudaFree would: nothing may still read the packed set
+    famsa::cache_free(ctx->d_stream); famsa::cache_free(ctx->d_tables); famsa::cache_free(ctx->d_len);
+    famsa::cache_free(ctx->d_toff); famsa::cache_free(ctx->d_goff);
     delete ctx;
 }
 
@@ -174,10 +230,11 @@ struct DevTmp {                       // pack_impl's scratch: ONE device allocat
     uint8_t* base = nullptr;          // per piece cost famsa_pack ~2 ms), freed on every exit path
     size_t cap = 0, used = 0;
     std::vector<void*> extra;         // pieces that did not fit the reservation (never with the sizes pack_impl reserves)
-    ~DevTmp() { cudaFree(base); for (void* p : extra) cudaFree(p); }
+    int device = 0;
+    ~DevTmp() { cudaDeviceSynchronize(); famsa::cache_free(base); for (void* p : extra) famsa::cache_free(p); }
     static size_t padded(size_t bytes) { return (std::max<size_t>(bytes, 1) + 255) & ~(size_t)255; }
     int reserve(size_t bytes) {
-        cudaError_t e = cudaMalloc((void**)&base, std::max<size_t>(bytes, 256));
+        cudaError_t e = famsa::cache_alloc(device, (void**)&base, std::max<size_t>(bytes, 256));
         if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); famsa::set_error("famsa_pack: device allocation failed"); return FAMSA_ENOMEM; }
         if (e != cudaSuccess) return famsa::cuda_fail(e, "cudaMalloc");
         cap = std::max<size_t>(bytes, 256);
@@ -186,15 +243,15 @@ struct DevTmp {                       // pack_impl's scratch: ONE device allocat
     template <typename T> int alloc(T** p, size_t n) {
         const size_t bytes = padded(n * sizeof(T));
         if (used + bytes <= cap) { *p = reinterpret_cast<T*>(base + used); used += bytes; return FAMSA_OK; }
-        cudaError_t e = famsa::dalloc(p, n);
+        cudaError_t e = famsa::dalloc(device, p, n);
         if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); famsa::set_error("famsa_pack: device allocation failed"); return FAMSA_ENOMEM; }
         if (e != cudaSuccess) return famsa::cuda_fail(e, "cudaMalloc");
         extra.push_back(*p);
         return FAMSA_OK;
     }
 };
-template <typename T> int ctx_alloc(T** p, size_t n) {
-    cudaError_t e = famsa::dalloc(p, n);
+template <typename T> int ctx_alloc(int device, T** p, size_t n) {
+    cudaError_t e = famsa::dalloc(device, p, n);
     if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); famsa::set_error("famsa_pack: device allocation failed"); return FAMSA_ENOMEM; }
     if (e != cudaSuccess) return famsa::cuda_fail(e, "cudaMalloc");
     return FAMSA_OK;
@@ -227,6 +284,7 @@ static int pack_impl(const uint8_t* seqs, const int64_t* offsets, int64_t k, int
     auto ms_since = [](clk::time_point t) { return std::chrono::duration<double, std::milli>(clk::now() - t).count(); };
     clk::time_point t_phase = clk::now();
     DevTmp tmp;
+    tmp.device = device;
     cudaStream_t st = nullptr;           // legacy default stream; pack synchronises before returning
     size_t cub_bytes = 0;
     if (k > 0) FAMSA_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, cub_bytes, (uint32_t*)nullptr, (uint32_t*)nullptr, (uint32_t*)nullptr,
@@ -312,11 +370,11 @@ static int pack_impl(const uint8_t* seqs, const int64_t* offsets, int64_t k, int
     // ---- device-resident set
     uint32_t* d_twords = nullptr;
     FAMSA_TRY(tmp.alloc(&d_twords, twords.size()));
-    FAMSA_TRY(ctx_alloc(&ctx->d_stream, ctx->stream_bytes + 512));
-    FAMSA_TRY(ctx_alloc(&ctx->d_tables, ctx->table_bytes / 4 + 64));
-    FAMSA_TRY(ctx_alloc(&ctx->d_len, (size_t)k));
-    FAMSA_TRY(ctx_alloc(&ctx->d_toff, (size_t)k));
-    FAMSA_TRY(ctx_alloc(&ctx->d_goff, (size_t)ctx->n_groups + 1));
+    FAMSA_TRY(ctx_alloc(device, &ctx->d_stream, ctx->stream_bytes + 512));
+    FAMSA_TRY(ctx_alloc(device, &ctx->d_tables, ctx->table_bytes / 4 + 64));
+    FAMSA_TRY(ctx_alloc(device, &ctx->d_len, (size_t)k));
+    FAMSA_TRY(ctx_alloc(device, &ctx->d_toff, (size_t)k));
+    FAMSA_TRY(ctx_alloc(device, &ctx->d_goff, (size_t)ctx->n_groups + 1));
     if (k > 0) {
         FAMSA_CUDA(cudaMemcpyAsync(ctx->d_len, ctx->len.data(), sizeof(uint32_t) * k, cudaMemcpyHostToDevice, st));
         FAMSA_CUDA(cudaMemcpyAsync(ctx->d_toff, ctx->toff.data(), sizeof(uint32_t) * k, cudaMemcpyHostToDevice, st));

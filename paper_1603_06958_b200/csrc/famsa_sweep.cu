@@ -552,6 +552,7 @@ extern "C" int famsa_trim(void) {
     std::vector<Staging*> all;
     { std::lock_guard<std::mutex> lk(g_pool_mu); all.swap(g_pool); }
     for (Staging* s : all) staging_destroy(s);
+    cache_trim();
     return FAMSA_OK;
 }
 
