@@ -86,11 +86,13 @@ __device__ __forceinline__ unsigned long long cand_key(float w, uint32_t other) 
 __device__ __forceinline__ uint32_t key_other(unsigned long long key) { return ~(uint32_t)key; }
 __device__ __forceinline__ uint32_t key_wbits1(unsigned long long key) { return (uint32_t)(key >> 32); }
 
-// ---- round-0 candidates from a caller's block (famsa_tree_update): one pass, both directions -----------
-// Best entry of each block row v over its columns u < v.  One CTA per row, 4 independent loads in flight per
-// thread (measured r01: 1024 CTAs read a 1.7 GB block at 5.7 TB/s).
-__global__ void __launch_bounds__(256) tree_cand_row_kernel(const float* __restrict__ sim, uint32_t i0, uint32_t i1, int64_t out_base,
-                                                            unsigned long long* __restrict__ cand_row) {
+// ---- round-0 candidates from a caller's block (famsa_tree_update): ONE pass, both directions -----------
+// One CTA per block row v, 4 independent loads in flight per thread (measured r01: 1024 CTAs read a 1.7 GB block at
+// 5.7 TB/s).  The row's best entry is reduced in the CTA; every entry is also a candidate of its COLUMN u, offered to
+// cand_col[u] through the monotone filter (a plain read of the L2-resident key, an atomicMax only if it improves), as
+// the sweep's epilogue does in the fused pipeline.  The caller zeroes cand_col[0, i1) first.
+__global__ void __launch_bounds__(256) tree_cand_kernel(const float* __restrict__ sim, uint32_t i0, uint32_t i1, int64_t out_base,
+                                                        unsigned long long* __restrict__ cand_row, unsigned long long* __restrict__ cand_col) {
     const uint32_t v = i0 + blockIdx.x;
     const float* row = sim + ((int64_t)v * (v - 1) / 2 - out_base);
     float bw = -1.0f; uint32_t bo = 0xFFFFFFFFu;
@@ -98,6 +100,8 @@ __global__ void __launch_bounds__(256) tree_cand_row_kernel(const float* __restr
     for (uint32_t u = threadIdx.x; u < v; u += 256) {
         const float w = __ldg(row + u);
         if (w > bw) { bw = w; bo = u; }                    // u ascends per thread: the first of equals stays
+        const unsigned long long ck = cand_key(w, v);
+        if (ck > cand_col[u]) atomicMax(cand_col + u, ck);
     }
     unsigned long long key = bo == 0xFFFFFFFFu ? 0ull : cand_key(bw, bo);
 #pragma unroll
@@ -109,32 +113,6 @@ __global__ void __launch_bounds__(256) tree_cand_row_kernel(const float* __restr
 #pragma unroll
         for (int q = 1; q < 8; ++q) key = max(key, sk[q]);
         cand_row[v] = key;
-    }
-}
-
-// Best entry of each column u < i1-1 over the block's rows v > u.  A CTA covers 64 consecutive columns with 8
-// row slices (threadIdx.y): consecutive threads read consecutive floats of a row (coalesced).
-constexpr int COL_X = 64, COL_Y = 8;
-__global__ void __launch_bounds__(COL_X * COL_Y) tree_cand_col_kernel(const float* __restrict__ sim, uint32_t i0, uint32_t i1, int64_t out_base,
-                                                                      unsigned long long* __restrict__ cand_col) {
-    __shared__ unsigned long long sk[COL_Y][COL_X];
-    const uint32_t u = blockIdx.x * COL_X + threadIdx.x;
-    const bool live = u + 1 < i1;
-    float bw = -1.0f; uint32_t bo = 0xFFFFFFFFu;
-    if (live) {
-#pragma unroll 4
-        for (uint32_t v = max(i0, u + 1) + threadIdx.y; v < i1; v += COL_Y) {
-            const float w = __ldg(sim + ((int64_t)v * (v - 1) / 2 - out_base + u));
-            if (w > bw) { bw = w; bo = v; }                // v ascends within a slice
-        }
-    }
-    sk[threadIdx.y][threadIdx.x] = bo == 0xFFFFFFFFu ? 0ull : cand_key(bw, bo);
-    __syncthreads();
-    if (threadIdx.y == 0 && live) {
-        unsigned long long key = sk[0][threadIdx.x];
-#pragma unroll
-        for (int q = 1; q < COL_Y; ++q) key = max(key, sk[q][threadIdx.x]);
-        cand_col[u] = key;
     }
 }
 
@@ -381,9 +359,9 @@ int tree_consume(famsa_tree* t, int64_t i0, int64_t i1, const float* sim, int64_
     const BlockArgs a = block_args(t, i0, i1, slot);
     const unsigned gv = (unsigned)((i1 + 255) / 256);
     if (!fused) {
-        tree_cand_row_kernel<<<(unsigned)(i1 - i0), 256, 0, st>>>(sim, a.i0, a.i1, out_base, t->cand_row[slot]);
-        if (i1 >= 2) tree_cand_col_kernel<<<(unsigned)((i1 - 1 + COL_X - 1) / COL_X), dim3(COL_X, COL_Y), 0, st>>>(sim, a.i0, a.i1, out_base, t->cand_col[slot]);
-        t->launches += 2;
+        FAMSA_CUDA(cudaMemsetAsync(t->cand_col[slot], 0, sizeof(unsigned long long) * (size_t)i1, st));
+        tree_cand_kernel<<<(unsigned)(i1 - i0), 256, 0, st>>>(sim, a.i0, a.i1, out_base, t->cand_row[slot], t->cand_col[slot]);
+        t->launches += 1;
     }
     tree_pick_kernel<<<gv, 256, 0, st>>>(a);
     tree_hook0_kernel<<<gv, 256, 0, st>>>(a);
