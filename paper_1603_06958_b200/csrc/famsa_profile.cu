@@ -7,8 +7,9 @@
 // previous profile column (row) in registers: 3 J floats.  The rows are swept in a skewed wavefront: at step t
 // lane l computes row t - l + 1, so what it needs from the left -- the three states of lane l-1's last residue
 // in the same row -- was produced one step earlier and arrives by one __shfl_up per state; the value received
-// for the previous row is kept as the diagonal.  Per cell: one L1-resident load of cost[row][residue] and ~25
-// fp32 adds / compares / selects, one direction byte (2 bits per state).  All arithmetic is fp32 adds,
+// for the previous row is kept as the diagonal.  Per cell: one shared-memory load of cost[row][residue] (the rows
+// stream through a per-warp ring, one coalesced global load per step) and ~25 fp32 adds / compares / selects, one
+// direction byte (2 bits per state).  All arithmetic is fp32 adds,
 // subtractions and comparisons in the order the oracle's fp32 mode uses (products of nseq and a gap cost are
 // formed once with __fmul_rn, nothing can contract into an FMA), so scores AND traceback decisions are
 // bit-identical to it.  A second kernel (one thread per alignment) walks the direction bytes back.
@@ -23,11 +24,13 @@
 namespace famsa {
 
 constexpr float NEG = -3.0e38f;
+constexpr int RING_ROWS = 64, RING_STRIDE = 33;              // per-warp ring of cost rows in shared memory (floats)
+constexpr size_t RING_BYTES = 4 * RING_ROWS * RING_STRIDE * sizeof(float);   // 4 warps per CTA
 
 struct AlignDesc {
     int64_t cost_row0;       // first cost row of the profile
     int64_t seq0;            // first residue of the sequence
-    int64_t dir0;            // byte offset of the direction matrix in the workspace (row stride 32 J)
+    int64_t dir0;            // byte offset of the direction bytes in the workspace (n1 + 31 skewed rows of 32 J bytes)
     int64_t path_end;        // end of the path segment
     int32_t n1, n2, idx, j;  // columns, residues, index in the batch, residues per lane
 };
@@ -73,19 +76,32 @@ __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restric
     float x0 = 0.0f;                                         // lane 0: X[i][0], columns before the first residue
     float rM = NEG, rX = NEG, rY = NEG;                      // the row this lane finished last, at its last residue
     const float* crow = cost + d.cost_row0 * SYMS;
+    // Cost rows go through a per-warp ring in shared memory: at one step the 32 lanes work on 32 DIFFERENT profile
+    // columns, so a direct load of cost[column][residue] touches 32 cache lines per instruction and the L1 pipeline
+    // -- not the ALU -- sets the pace (measured r02: 2.5 of 3 warps per scheduler waiting on the long scoreboard).
+    // Instead the warp loads ONE new row per step with a single coalesced 128-byte load and the lanes read their
+    // values from the ring; rows are 33 words apart, so the bank of (row r, symbol c) is (r + c) mod 32 and lanes on
+    // different rows with the same residue do not collide systematically.
+    extern __shared__ float ring_all[];
+    float* ring = ring_all + (threadIdx.x >> 5) * (RING_ROWS * RING_STRIDE);
+    ring[lane] = crow[lane];                                 // row 0 (n1 >= 1)
+    __syncwarp();
     uint8_t* dir = ws + d.dir0;
     const int stride = 32 * J;
     const int steps = n1 + 31;
     for (int t = 0; t < steps; ++t) {
         const int i = t - lane + 1;
+        const float next_row = t + 1 < n1 ? __ldg(crow + (size_t)(t + 1) * SYMS + lane) : 0.0f;   // cost row t+1, used from the next step on
         float lM = __shfl_up_sync(0xffffffffu, rM, 1), lX = __shfl_up_sync(0xffffffffu, rX, 1), lY = __shfl_up_sync(0xffffffffu, rY, 1);
-        if (i < 1 || i > n1) continue;                       // (no shuffle below this line)
+        if (i >= 1 && i <= n1) {
         if (lane == 0) { x0 = i == 1 ? 0.0f - To : x0 - Te; lM = NEG; lX = x0; lY = NEG; }
         const float goy = i == n1 ? nTo : nGo, gey = i == n1 ? nTe : nGe;
-        const float* ci = crow + (size_t)(i - 1) * SYMS;
+        const float* ci = ring + ((i - 1) & (RING_ROWS - 1)) * RING_STRIDE;
         float cM = dM, cX = dX, cY = dY;                     // diagonal of the lane's first residue
         dM = lM; dX = lX; dY = lY;                           // ... and the next row's
-        uint32_t dword = 0;
+        uint32_t dw[J / 4];
+#pragma unroll
+        for (int q = 0; q < J / 4; ++q) dw[q] = 0;
 #pragma unroll
         for (int c = 0; c < J; ++c) {
             const int j = j0 + c + 1;
@@ -94,7 +110,7 @@ __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restric
             float bst = cM, v; uint32_t from = 0, dd;
             if (cX > bst) { bst = cX; from = 1; }
             if (cY > bst) { bst = cY; from = 2; }
-            const float m = bst + __ldg(ci + code); dd = from;
+            const float m = bst + ci[code]; dd = from;
             bst = Mp[c] - gox; from = 0;
             v = Xp[c] - gex; if (v > bst) { bst = v; from = 1; }
             v = Yp[c] - gox; if (v > bst) { bst = v; from = 2; }
@@ -106,11 +122,7 @@ __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restric
             cM = Mp[c]; cX = Xp[c]; cY = Yp[c];
             Mp[c] = m; Xp[c] = x; Yp[c] = y;
             lM = m; lX = x; lY = y;
-            dword |= dd << (8 * (c & 3));
-            if ((c & 3) == 3) {
-                if (want_dir) *reinterpret_cast<uint32_t*>(dir + (size_t)(i - 1) * stride + j0 + c - 3) = dword;
-                dword = 0;
-            }
+            dw[c >> 2] |= dd << (8 * (c & 3));
             if (i == n1 && j == n2) {                        // the end cell: score and the state the walk starts in
                 float best = m; uint32_t st = 0;
                 if (x > best) { best = x; st = 1; }
@@ -119,6 +131,24 @@ __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restric
             }
         }
         rM = lM; rX = lX; rY = lY;
+        // Direction bytes in a SKEWED layout: the bytes of (row i, lane l) go to workspace row t = i - 1 + l, so that
+        // at one step all lanes write into the same 32 J-byte row (coalesced) instead of into 32 different rows.
+        if (want_dir) {
+            uint8_t* out = dir + (size_t)t * stride + j0;
+            if (J % 16 == 0) {
+#pragma unroll
+                for (int q = 0; q < J / 16; ++q) reinterpret_cast<uint4*>(out)[q] = make_uint4(dw[4 * q], dw[4 * q + 1], dw[4 * q + 2], dw[4 * q + 3]);
+            } else if (J % 8 == 0) {
+#pragma unroll
+                for (int q = 0; q < J / 8; ++q) reinterpret_cast<uint2*>(out)[q] = make_uint2(dw[2 * q], dw[2 * q + 1]);
+            } else {
+#pragma unroll
+                for (int q = 0; q < J / 4; ++q) reinterpret_cast<uint32_t*>(out)[q] = dw[q];
+            }
+        }
+        }
+        ring[((t + 1) & (RING_ROWS - 1)) * RING_STRIDE + lane] = next_row;     // the slot's old row (t - 63) was last read at step t - 32
+        __syncwarp();
     }
 }
 
@@ -136,7 +166,7 @@ __global__ void seqprof_trace_kernel(const AlignDesc* __restrict__ desc, int n, 
     uint8_t* out = path + d.path_end;
     while (i > 0 || j > 0) {
         uint32_t dd;
-        if (i > 0 && j > 0) dd = dir[(size_t)(i - 1) * stride + (j - 1)];
+        if (i > 0 && j > 0) dd = dir[(size_t)(i - 1 + (j - 1) / d.j) * stride + (j - 1)];   // skewed rows: see seqprof_kernel
         else if (i == 0) dd = (j == 1 ? 0u : 2u) << 4;        // row 0: a run of terminal gap columns
         else dd = (i == 1 ? 0u : 1u) << 2;                    // residue 0: a run of terminal gaps
         *--out = (uint8_t)st; ++len;
@@ -182,7 +212,7 @@ extern "C" int64_t famsa_seqprof_workspace(const int64_t* col_off_host, const in
     if (seqprof_check(col_off_host, seq_off_host, n_align, "famsa_seqprof_workspace") != FAMSA_OK) return -1;
     int64_t bytes = 0;
     for (int64_t b = 0; b < n_align; ++b)
-        bytes += (col_off_host[b + 1] - col_off_host[b]) * 32 * lanes_j(seq_off_host[b + 1] - seq_off_host[b]);
+        bytes += (col_off_host[b + 1] - col_off_host[b] + 31) * 32 * lanes_j(seq_off_host[b + 1] - seq_off_host[b]);
     return bytes + n_align;                                  // + one final-state byte per alignment
 }
 
@@ -206,7 +236,7 @@ extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off
         d.cost_row0 = col_off_host[b]; d.seq0 = seq_off_host[b];
         d.n1 = (int32_t)(col_off_host[b + 1] - col_off_host[b]); d.n2 = (int32_t)(seq_off_host[b + 1] - seq_off_host[b]);
         d.idx = (int32_t)b; d.j = lanes_j(d.n2);
-        d.dir0 = dir_bytes; dir_bytes += (int64_t)d.n1 * 32 * d.j;
+        d.dir0 = dir_bytes; dir_bytes += ((int64_t)d.n1 + 31) * 32 * d.j;   // n1 + 31 wavefront steps
         d.path_end = col_off_host[b + 1] + seq_off_host[b + 1];
         order[(size_t)b] = b;
     }
@@ -232,10 +262,10 @@ extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off
         while (g1 < n_align && sorted[(size_t)g1].j == sorted[(size_t)g0].j) ++g1;
         const int n = (int)(g1 - g0);
         const unsigned grid = (unsigned)((n + 3) / 4);       // 4 warps = 4 alignments per CTA
-#define SEQPROF_CASE(JJ) case JJ: seqprof_kernel<JJ><<<grid, 128, 0, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
+#define SEQPROF_CASE(JJ) case JJ: seqprof_kernel<JJ><<<grid, 128, RING_BYTES, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
         switch (sorted[(size_t)g0].j) {
             SEQPROF_CASE(4) SEQPROF_CASE(8) SEQPROF_CASE(12) SEQPROF_CASE(16) SEQPROF_CASE(20) SEQPROF_CASE(24) SEQPROF_CASE(28)
-            default: seqprof_kernel<32><<<grid, 128, 0, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
+            default: seqprof_kernel<32><<<grid, 128, RING_BYTES, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
         }
 #undef SEQPROF_CASE
         g0 = g1;
