@@ -50,6 +50,12 @@ __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restric
                                                       const uint8_t* __restrict__ seq, const float* __restrict__ gaps,
                                                       const int32_t* __restrict__ nseq, float* __restrict__ score,
                                                       uint8_t* __restrict__ final_state, uint8_t* __restrict__ ws, int want_dir) {
+    // The residues-per-lane groups of one batch are launched back to back as programmatic dependents: a group
+    // rarely fills the GPU (a batch of 8192 alignments splits into 8 groups), so the next group's CTAs start as soon
+    // as this group's are all resident.  The groups are independent (disjoint outputs); every working warp ends with
+    // griddepcontrol.wait, so a group cannot complete before its predecessor and the traceback kernel -- an
+    // ordinary launch after the last group -- sees all of them.
+    asm volatile("griddepcontrol.launch_dependents;");
     const int warp = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
     if (warp >= n) return;
     const AlignDesc d = desc[warp];
@@ -150,6 +156,7 @@ __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restric
         ring[((t + 1) & (RING_ROWS - 1)) * RING_STRIDE + lane] = next_row;     // the slot's old row (t - 63) was last read at step t - 32
         __syncwarp();
     }
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 // One thread per alignment walks the direction bytes from (n1, n2) back to (0, 0); the operations are written
@@ -242,7 +249,7 @@ extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off
     }
     std::stable_sort(order.begin(), order.end(), [&](int64_t p, int64_t q) {
         const AlignDesc &a = desc[(size_t)p], &c = desc[(size_t)q];
-        return a.j != c.j ? a.j < c.j : a.n1 > c.n1;
+        return a.j != c.j ? a.j > c.j : a.n1 > c.n1;            // heaviest group first, lighter groups fill its tail
     });
     std::vector<AlignDesc> sorted((size_t)n_align);
     for (int64_t b = 0; b < n_align; ++b) sorted[(size_t)b] = desc[(size_t)order[(size_t)b]];
@@ -262,11 +269,21 @@ extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off
         while (g1 < n_align && sorted[(size_t)g1].j == sorted[(size_t)g0].j) ++g1;
         const int n = (int)(g1 - g0);
         const unsigned grid = (unsigned)((n + 3) / 4);       // 4 warps = 4 alignments per CTA
-#define SEQPROF_CASE(JJ) case JJ: seqprof_kernel<JJ><<<grid, 128, RING_BYTES, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
+#define SEQPROF_CASE(JJ) case JJ: le = cudaLaunchKernelEx(&cfg, seqprof_kernel<JJ>, (const AlignDesc*)(d_desc + g0), n, cost_dev, seq_dev, gaps_dev, \
+                                                          nseq_dev, score_dev, final_state, ws, want_dir); break;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = RING_BYTES; cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        cudaError_t le = cudaSuccess;
         switch (sorted[(size_t)g0].j) {
             SEQPROF_CASE(4) SEQPROF_CASE(8) SEQPROF_CASE(12) SEQPROF_CASE(16) SEQPROF_CASE(20) SEQPROF_CASE(24) SEQPROF_CASE(28)
-            default: seqprof_kernel<32><<<grid, 128, RING_BYTES, st>>>(d_desc + g0, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir); break;
+            default: le = cudaLaunchKernelEx(&cfg, seqprof_kernel<32>, (const AlignDesc*)(d_desc + g0), n, cost_dev, seq_dev, gaps_dev,
+                                             nseq_dev, score_dev, final_state, ws, want_dir); break;
         }
+        FAMSA_CUDA(le);
 #undef SEQPROF_CASE
         g0 = g1;
     }
