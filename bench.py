@@ -598,8 +598,12 @@ def run_cuda(args, rank, world, local_rank):
     achieved = cells_step * args.steps * ALU_INSTR_PER_CELL / (ms_rank * 1e-3)   # this rank's stream
     peaks_file = os.path.join(ROOT, "MEASURED_PEAKS.json")
     sm_max = 1965.0
+    hbm_gbs, hbm_src = 6650.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
     if os.path.exists(peaks_file):
-        sm_max = float(json.load(open(peaks_file)).get("sm_max_mhz", sm_max))
+        peaks = json.load(open(peaks_file))
+        sm_max = float(peaks.get("sm_max_mhz", sm_max))
+        if peaks.get("hbm_gbs"):
+            hbm_gbs, hbm_src = float(peaks["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
     nominal = sm_count * 64 * sm_max * 1e6
     out_bytes = pairs_step * (2 + (4 if want_sim else 0))
     traffic = None
@@ -645,6 +649,8 @@ def run_cuda(args, rank, world, local_rank):
         "cpu_baseline": cpu,
         "cpu_bitparallel": cpu_bp,
         "output_gb_per_s": pairs_all * args.steps * (2 + (4 if want_sim else 0)) / sec / 1e9,
+        "output_frac_of_hbm_peak": pairs_all * args.steps * (2 + (4 if want_sim else 0)) / sec / 1e9 / (hbm_gbs * world),
+        "hbm_peak_gb_per_s": hbm_gbs, "hbm_peak_source": hbm_src,
     }
     if full is not None:
         line["full_sweep"] = full
