@@ -673,6 +673,10 @@ def run_seqprof(args, rank, world, local_rank):
     arrays with the scores, paths and path lengths read back.  Metric: DP cells (n1 x n2) per second."""
     import torch
     from paper_1603_06958_b200 import famsa as F, synth
+    dist = None
+    if world > 1:                      # alignments are independent (PAPER.md:107): every rank takes its own batch, no collective
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     B = args.batch
@@ -696,6 +700,8 @@ def run_seqprof(args, rank, world, local_rank):
         F.famsa_seqprof_align(cost, col_off, src["seq"], seq_off, src["gaps"], src["nseq"], score, path, plen, ws, stream)
     for _ in range(args.warmup):
         step(d)
+    if dist is not None:
+        dist.barrier()
     torch.cuda.synchronize()
     sampler = ClockSampler(local_rank); sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -703,16 +709,19 @@ def run_seqprof(args, rank, world, local_rank):
     for _ in range(args.steps):
         step(d)
     e1.record(stream)
+    if dist is not None:
+        dist.barrier()
     torch.cuda.synchronize()
     clocks = sampler.stop()
-    ms = e0.elapsed_time(e1)
-    value = cells * args.steps / ms / 1e6
+    ms_rank = e0.elapsed_time(e1)
+    ms, cells_all, _ = reduce_over_ranks(dist, ms_rank, cells, B, dev)      # max time over ranks, sum of the cells
+    value = cells_all * args.steps / ms / 1e6
     peak = F.famsa_alu_peak(local_rank)
     # Roofline: the ALU pipe.  Per cell and state: 2 compares + 2 value selects + 2 direction selects on
     # the ALU pipe (18 per cell; the 7 fp32 adds / subtracts run on the FMA pipe beside them).
     alu_per_cell = 18.0
-    roofline = {"bound": "alu", "achieved": cells * args.steps * alu_per_cell / (ms * 1e-3) / 1e12, "peak": peak["instr_per_s"] / 1e12,
-                "unit": "TIOP/s (ALU-pipe lane-instr)", "frac": cells * args.steps * alu_per_cell / (ms * 1e-3) / peak["instr_per_s"],
+    roofline = {"bound": "alu", "achieved": cells * args.steps * alu_per_cell / (ms_rank * 1e-3) / 1e12, "peak": peak["instr_per_s"] / 1e12,
+                "unit": "TIOP/s (ALU-pipe lane-instr)", "frac": cells * args.steps * alu_per_cell / (ms_rank * 1e-3) / peak["instr_per_s"],
                 "traffic": None, "algorithmic_instr_per_cell": alu_per_cell, "kernel": "famsa::seqprof_kernel<J>",
                 "peak_source": "famsa_alu_peak micro-kernel, measured in this run",
                 "note": "padding of n2 to 32 J lane slots, the 31-step skew of the wavefront and the traceback all count against the kernel"}
@@ -729,6 +738,13 @@ def run_seqprof(args, rank, world, local_rank):
     for _ in range(args.steps):
         e2e_step()
     e2e_sec = time.perf_counter() - t0
+    if dist is not None:
+        tt = torch.tensor([e2e_sec], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_sec = float(tt.item())
+        dist.destroy_process_group()
+    if rank != 0:
+        return
     # the oracle beside it and against it: a bounded sample of the batch (fp32 mode: same-precision decisions)
     cpu = parity = None
     if not args.no_cpu and rank == 0:
@@ -753,9 +769,9 @@ def run_seqprof(args, rank, world, local_rank):
             "config": {"workload": "SURVEY 8(f) NEXT-4: %d independent sequence-vs-profile alignments per step (profiles of 100-700 columns from 1-40 "
                                    "sequences, sequences with indels), costs + DP + traceback" % B,
                        "cells_per_step": cells, "l2": "direction matrices (%.2f GB per step) exceed L2" % (ws.numel() / 1e9)},
-            "alignments_per_s": B * args.steps / ms * 1e3,
+            "alignments_per_s": B * world * args.steps / ms * 1e3,
             "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"], "samples": clocks["samples"]},
-            "e2e": {"value": cells * args.steps / e2e_sec / 1e9, "unit": UNIT,
+            "e2e": {"value": cells_all * args.steps / e2e_sec / 1e9, "unit": UNIT,
                     "h2d_bytes_per_step": int(sum(v.numel() * v.element_size() for v in h.values())),
                     "d2h_bytes_per_step": int(h_score.numel() * 4 + h_path.numel() + h_plen.numel() * 4)},
             "gpu_launches": 10 * args.steps, "roofline": roofline, "cpu_baseline": cpu, "parity_in_bench": parity}
