@@ -16,6 +16,7 @@
 // (Tried, r02: loading the lane's cost values one row ahead -- +16 registers at J = 16 -- was 1 % slower.)
 #include <algorithm>
 #include <cmath>
+#include <mutex>
 #include <vector>
 
 #include "famsa_internal.h"
@@ -185,6 +186,14 @@ __global__ void seqprof_trace_kernel(const AlignDesc* __restrict__ desc, int n, 
 }
 
 // residues per lane: the smallest multiple of 4 with 32 J >= n2 (4 .. 32), so at most 127 of the 32 J lane slots idle
+// Pinned staging for the descriptors of a call: two buffers used alternately, each guarded by an event recorded
+// after its copy, so that a call neither synchronises the stream (a cudaMemcpyAsync from pageable memory would) nor
+// waits for more than the call before the previous one: consecutive batches overlap host preparation with the GPU.
+struct DescStage { AlignDesc* p = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; bool used = false; };
+static std::mutex g_desc_mu;
+static DescStage g_desc[2];
+static int g_desc_next = 0;
+
 static int lanes_j(int64_t n2) { return (int)(4 * ((n2 + 127) / 128)); }
 
 }  // namespace famsa
@@ -251,7 +260,19 @@ extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off
         const AlignDesc &a = desc[(size_t)p], &c = desc[(size_t)q];
         return a.j != c.j ? a.j > c.j : a.n1 > c.n1;            // heaviest group first, lighter groups fill its tail
     });
-    std::vector<AlignDesc> sorted((size_t)n_align);
+    std::lock_guard<std::mutex> desc_lock(g_desc_mu);
+    DescStage& stg = g_desc[g_desc_next]; g_desc_next ^= 1;
+    if (!stg.ev) FAMSA_CUDA(cudaEventCreateWithFlags(&stg.ev, cudaEventDisableTiming));
+    if (stg.used) FAMSA_CUDA(cudaEventSynchronize(stg.ev));              // the copy out of this buffer two calls ago
+    if (stg.cap < (size_t)n_align) {
+        if (stg.p) cudaFreeHost(stg.p);
+        stg.p = nullptr; stg.cap = 0;
+        if (cudaMallocHost((void**)&stg.p, sizeof(AlignDesc) * (size_t)n_align) != cudaSuccess) {
+            cudaGetLastError(); set_error("famsa_seqprof_align: pinned allocation failed"); return FAMSA_ENOMEM;
+        }
+        stg.cap = (size_t)n_align;
+    }
+    AlignDesc* sorted = stg.p;
     for (int64_t b = 0; b < n_align; ++b) sorted[(size_t)b] = desc[(size_t)order[(size_t)b]];
     uint8_t* final_state = nullptr;
     uint8_t* ws = static_cast<uint8_t*>(workspace_dev);
@@ -260,8 +281,9 @@ extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off
     FAMSA_CUDA(cudaMallocAsync((void**)&d_desc, sizeof(AlignDesc) * (size_t)n_align, st));
     if (ws) final_state = ws + dir_bytes;
     else { FAMSA_CUDA(cudaMallocAsync((void**)&own_state, (size_t)n_align, st)); final_state = own_state; }
-    FAMSA_CUDA(cudaMemcpyAsync(d_desc, sorted.data(), sizeof(AlignDesc) * (size_t)n_align, cudaMemcpyHostToDevice, st));
-    FAMSA_CUDA(cudaStreamSynchronize(st));                   // `sorted` is pageable and dies with this call
+    FAMSA_CUDA(cudaMemcpyAsync(d_desc, sorted, sizeof(AlignDesc) * (size_t)n_align, cudaMemcpyHostToDevice, st));
+    FAMSA_CUDA(cudaEventRecord(stg.ev, st));
+    stg.used = true;
     const int want_dir = path_dev != nullptr;
     int64_t g0 = 0;
     while (g0 < n_align) {
