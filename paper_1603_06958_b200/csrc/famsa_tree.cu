@@ -178,35 +178,42 @@ __global__ void tree_cid_kernel(BlockArgs a) {
 }
 
 // The one pass over the block: K[row][component b] = best edge from block row v into component b != comp(v).
-// One CTA per row.  The table row (P x 8 B <= 8 KB) stays in L1/L2; an entry is read with a plain load and
-// only an improving key goes to atomicMax (a stale read only costs a redundant atomic).  HBM-bound: one
-// read of the block + 2 B of (L2-resident) component id per entry.
+// One CTA per row, so the row's table (P x 8 B <= 8 KB) is PRIVATE to the CTA: it lives in shared memory, an entry is
+// read with a plain load and only an improving key goes to a shared-memory atomicMax (a stale read only costs a
+// redundant atomic), and the CTA writes its P entries out once at the end -- no global atomics, no gathers from
+// global memory.  HBM-bound: one read of the block + 2 B of (L2-resident) component id per entry.
 __global__ void __launch_bounds__(256) tree_rowcomp_kernel(const float* __restrict__ sim, uint32_t i0, uint32_t i1, int64_t out_base, BlockArgs a) {
-    if (a.st->P <= 1) return;                               // the block graph is already connected
+    __shared__ unsigned long long sk[KSTRIDE];
+    const uint32_t P = a.st->P;
+    if (P <= 1) return;                                     // the block graph is already connected
+    for (uint32_t b = threadIdx.x; b < P; b += 256) sk[b] = 0ull;
+    __syncthreads();
     const uint32_t v = i0 + blockIdx.x;
     const float* row = sim + ((int64_t)v * (v - 1) / 2 - out_base);
     const uint16_t ca = a.cid16[v];
-    unsigned long long* krow = a.ktab + (size_t)blockIdx.x * KSTRIDE;
     const uint16_t* __restrict__ cid = a.cid16;
     uint32_t u = threadIdx.x;
-    for (; u + 768 < v; u += 1024) {                        // 4 independent loads in flight
-        float w[4]; uint16_t c[4];
+    for (; u + 7 * 256 < v; u += 8 * 256) {                 // 8 independent loads of each kind in flight
+        float w[8]; uint16_t c[8];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) { w[q] = __ldg(row + u + q * 256); c[q] = cid[u + q * 256]; }
+        for (int q = 0; q < 8; ++q) { w[q] = __ldg(row + u + q * 256); c[q] = cid[u + q * 256]; }
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
+        for (int q = 0; q < 8; ++q)
             if (c[q] != ca) {
                 const unsigned long long key = cand_key(w[q], u + q * 256);
-                if (key > krow[c[q]]) atomicMax(&krow[c[q]], key);
+                if (key > sk[c[q]]) atomicMax(&sk[c[q]], key);
             }
     }
     for (; u < v; u += 256) {
         const float w = __ldg(row + u); const uint16_t c = cid[u];
         if (c != ca) {
             const unsigned long long key = cand_key(w, u);
-            if (key > krow[c]) atomicMax(&krow[c], key);
+            if (key > sk[c]) atomicMax(&sk[c], key);
         }
     }
+    __syncthreads();
+    unsigned long long* krow = a.ktab + (size_t)blockIdx.x * KSTRIDE;
+    for (uint32_t b = threadIdx.x; b < P; b += 256) krow[b] = sk[b];
 }
 
 // S += the best entries of K per pair of components (ties keep several: harmless).
@@ -367,7 +374,6 @@ int tree_consume(famsa_tree* t, int64_t i0, int64_t i1, const float* sim, int64_
     tree_hook0_kernel<<<gv, 256, 0, st>>>(a);
     tree_root0_kernel<<<gv, 256, 0, st>>>(a);
     tree_cid_kernel<<<gv, 256, 0, st>>>(a);
-    FAMSA_CUDA(cudaMemsetAsync(t->ktab, 0, sizeof(unsigned long long) * (size_t)(i1 - i0) * KSTRIDE, st));
     FAMSA_CUDA(cudaMemsetAsync(t->wab, 0, sizeof(uint32_t) * (size_t)KSTRIDE * KSTRIDE, st));
     tree_rowcomp_kernel<<<(unsigned)(i1 - i0), 256, 0, st>>>(sim, a.i0, a.i1, out_base, a);
     const unsigned gk = (unsigned)(((size_t)(i1 - i0) * KSTRIDE + 255) / 256);
