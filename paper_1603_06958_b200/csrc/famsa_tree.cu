@@ -562,7 +562,8 @@ __global__ void tree_uf_init_kernel(uint32_t k, uint32_t* uf, unsigned long long
 //   D (all threads)  the local result goes back to the global arrays: every root of the batch points to its
 //                    final root, the final roots carry (cluster id, size), the endpoints are compressed.
 // Cluster ids and sizes are < 2^32 (k <= 2^31 - 16), so (id, size) is one 64-bit word.
-constexpr int DG_B = 128, DG_H = 512;
+constexpr int DG_B = 512, DG_H = 2048, DG_HBITS = 11;    // batch, hash-table size (2^DG_HBITS >= 4 x slots / 2); measured
+                                                          // r02: the per-batch costs (finds, hash, write-back) are ~60 % of a 128-edge batch
 __global__ void __launch_bounds__(DG_B) tree_dendrogram_kernel(uint32_t k, const uint32_t* __restrict__ order, const uint32_t* __restrict__ ta,
                                                                const uint32_t* __restrict__ tb, const float* __restrict__ tw,
                                                                uint32_t* uf, unsigned long long* info,
@@ -598,7 +599,7 @@ __global__ void __launch_bounds__(DG_B) tree_dendrogram_kernel(uint32_t k, const
         // B: canonical slots through the hash table; the canonical ones load their root's (id, size)
         for (uint32_t s = tid; s < 2 * nb; s += DG_B) {
             const uint32_t r = s_root[s];
-            uint32_t h = (r * 2654435761u) >> 23;           // 9 bits
+            uint32_t h = (r * 2654435761u) >> (32 - DG_HBITS);
             for (;;) {
                 const uint32_t old = atomicCAS(&h_key[h], 0xFFFFFFFFu, r);
                 if (old == 0xFFFFFFFFu || old == r) break;
@@ -679,8 +680,8 @@ extern "C" int famsa_tree_finish(famsa_tree* t, int64_t* id_a_host, int64_t* id_
     const size_t o_idx = carve(4ull * m), o_idx2 = carve(4ull * m), o_order = carve(4ull * m), o_uf = carve(4ull * k), o_info = carve(8ull * k);
     const size_t o_oa = carve(8ull * m), o_ob = carve(8ull * m), o_osz = carve(8ull * m), o_ow = carve(4ull * m), o_cub = carve(std::max(b1, b2));
     uint8_t* base = nullptr;
-    if (cudaMalloc((void**)&base, off) != cudaSuccess) { cudaGetLastError(); set_error("famsa_tree_finish: device allocation failed"); return FAMSA_ENOMEM; }
-    struct Guard { uint8_t* p; ~Guard() { cudaFree(p); } } guard{base};
+    if (cache_alloc(t->device, (void**)&base, off) != cudaSuccess) { cudaGetLastError(); set_error("famsa_tree_finish: device allocation failed"); return FAMSA_ENOMEM; }
+    struct Guard { uint8_t* p; ~Guard() { cudaDeviceSynchronize(); cache_free(p); } } guard{base};   // scratch from the block cache (famsa_trim releases it)
     unsigned long long *idk = (unsigned long long*)(base + o_idk), *idk2 = (unsigned long long*)(base + o_idk2), *info = (unsigned long long*)(base + o_info);
     uint32_t *wk = (uint32_t*)(base + o_wk), *wk2 = (uint32_t*)(base + o_wk2), *idx = (uint32_t*)(base + o_idx), *idx2 = (uint32_t*)(base + o_idx2);
     uint32_t *order = (uint32_t*)(base + o_order), *uf = (uint32_t*)(base + o_uf);
