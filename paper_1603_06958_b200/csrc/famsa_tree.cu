@@ -11,8 +11,8 @@
 //      one pass over the block (famsa_tree_update on a caller's block).  Every component of the pick graph
 //      contains a block row, so there are P <= rows <= 1024 components.
 //   2. ONE pass over the block fills K[row][component] = the best edge from each block row into each OTHER
-//      component (monotone filter: a plain read of the L1/L2-resident table entry, an atomicMax only when the
-//      entry improves, so atomics are ~ entries x ln(columns)).  The picks of 1. plus, per pair of
+//      component (one CTA per row keeps the row's table in shared memory; monotone filter: a plain read of the
+//      entry, an atomicMax only when it improves, so atomics are ~ entries x ln(columns)).  The picks of 1. plus, per pair of
 //      components, the best entries of K are a sparse edge set S with MSF(T u block) = MSF(T u S): an edge
 //      inside a component, or not the best of its component pair, closes a cycle of heavier edges.
 //   3. a persistent cooperative kernel merges S into T by Boruvka rounds over (T's edges + S) with grid-wide
