@@ -123,6 +123,24 @@ def test_guide_tree_end_to_end(F, oracle):
         assert size[-1] == k and np.all(np.diff(mw[~inf]) <= 0)
 
 
+def test_guide_tree_tiny_sets(F, oracle):
+    """famsa_guide_tree at the smallest sizes and block shapes (k = 2, 3, 5, 33; blocks of 1, 2, 1024 rows)."""
+    from oracle import slink_oracle as so
+    from paper_1603_06958_b200 import synth
+    for k in (2, 3, 5, 33):
+        seqs, offsets = synth.family(0, k=k, seed=300 + k)
+        _, sref = oracle.rows(seqs, offsets, 0, k)
+        heights = so.merge_heights(so.single_linkage(so.full_matrix(k, sref)))
+        for block in (1, 2, 1024):
+            with F.famsa_pack(seqs, offsets) as ctx:
+                ia, ib, mw, size = F.famsa_guide_tree(ctx, block)
+            mw = mw.astype(np.float64)
+            inf = np.isinf(heights)
+            assert mw.size == k - 1 and size[-1] == k and np.array_equal(np.isinf(mw), inf)
+            assert np.all(np.abs(mw[~inf] - heights[~inf]) <= 1e-6 * heights[~inf])
+            assert sorted(np.concatenate([ia, ib]).tolist()) == list(range(2 * k - 2))
+
+
 def feed_blocks(F, tri, k, blocks):
     import torch
     t = F.famsa_tree_create(k)
