@@ -113,6 +113,38 @@ def test_exact_inputs_ties_and_score_only(F):
         assert float(score[b]) == s64 and np.array_equal(path[end - plen[b]:end], p64)
 
 
+def test_back_to_back_calls_without_synchronisation(F):
+    """Three batches enqueued on one stream with no host synchronisation in between (the call stages its descriptors
+    through two pinned buffers): every batch's scores and paths equal the oracle's fp32 mode."""
+    import torch
+    from paper_1603_06958_b200 import synth
+    from oracle import profile_oracle as po
+    subst = synth.substitution_matrix()
+    d_subst = torch.from_numpy(subst).cuda()
+    jobs = []
+    for n, seed in ((9, 411), (17, 412), (5, 413)):
+        counts, col_off, seq, seq_off, nseq = synth.profile_batch(n, seed=seed, n1_range=(20, 300))
+        gaps = np.tile(BASE_GAPS, (n, 1))
+        cost = torch.empty((counts.shape[0], 32), dtype=torch.float32, device="cuda")
+        bufs = dict(cost=cost, counts=torch.from_numpy(counts.astype(np.int32)).cuda(), seq=torch.from_numpy(seq).cuda(),
+                    gaps=torch.from_numpy(gaps).cuda(), nseq=torch.from_numpy(nseq).cuda(),
+                    score=torch.empty(n, dtype=torch.float32, device="cuda"),
+                    path=torch.empty(int(col_off[-1] + seq_off[-1]), dtype=torch.uint8, device="cuda"),
+                    plen=torch.empty(n, dtype=torch.int32, device="cuda"),
+                    ws=torch.empty(F.famsa_seqprof_workspace(col_off, seq_off), dtype=torch.uint8, device="cuda"))
+        jobs.append((col_off, seq, seq_off, nseq, gaps, bufs))
+    for col_off, seq, seq_off, nseq, gaps, b in jobs:           # enqueue everything first
+        F.famsa_profile_costs(b["counts"], d_subst, b["cost"])
+        F.famsa_seqprof_align(b["cost"], col_off, b["seq"], seq_off, b["gaps"], b["nseq"], b["score"], b["path"], b["plen"], b["ws"])
+    torch.cuda.synchronize()
+    for col_off, seq, seq_off, nseq, gaps, b in jobs:
+        cost, score, path, plen = b["cost"].cpu().numpy(), b["score"].cpu().numpy(), b["path"].cpu().numpy(), b["plen"].cpu().numpy()
+        for q in range(col_off.size - 1):
+            s32, p32 = po.align(cost[col_off[q]:col_off[q + 1]], seq[seq_off[q]:seq_off[q + 1]], gaps[q], int(nseq[q]), want_path=True, precision="f32")
+            end = int(col_off[q + 1] + seq_off[q + 1])
+            assert score[q] == np.float32(s32) and np.array_equal(path[end - plen[q]:end], p32)
+
+
 def test_errors(F):
     import torch
     z = torch.zeros(64, dtype=torch.float32, device="cuda")
