@@ -72,6 +72,26 @@ int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off_host, cons
                         float* score_dev, uint8_t* path_dev, int32_t* path_len_dev, void* workspace_dev,
                         void* cuda_stream);
 
+#define FAMSA_SEQPROF_STATIC_MAX 16384   /* alignments per famsa_seqprof_scores_static call */
+
+/*
+ * famsa_seqprof_scores_static -- famsa_seqprof_align in score-only mode for callers that cannot allocate (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): the call makes NO cudaMalloc / cudaFree /
+ * cudaMallocAsync / cudaMallocHost call and no heap allocation.  Its scratch (the device copy of the alignment
+ * descriptors + one final-state byte per alignment) is a file-scope `static __device__` array of
+ * FAMSA_SEQPROF_STATIC_MAX x 49 bytes = 0.8 MB that every GPU which loads the library holds until the process exits.
+ * Arguments as famsa_seqprof_align (scores only: no path, no workspace); the CURRENT device is used; enqueued on
+ * cuda_stream.  Scores are bit-identical to famsa_seqprof_align's.
+ *   - n_align > FAMSA_SEQPROF_STATIC_MAX: FAMSA_ERANGE (split the batch or use famsa_seqprof_align).
+ *   - Every call on a device shares the one array, which keeps the previous call's contents; a call overwrites all it
+ *     reads, so calls ORDERED on the device (same stream, or ordered by events) are independent of one another, but
+ *     calls that OVERLAP on the GPU (different streams without ordering, several host threads on different streams)
+ *     RACE on it and give undefined scores.
+ */
+int famsa_seqprof_scores_static(const float* cost_dev, const int64_t* col_off_host, const uint8_t* seq_dev,
+                                const int64_t* seq_off_host, const float* gaps_dev, const int32_t* nseq_dev,
+                                int64_t n_align, float* score_dev, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

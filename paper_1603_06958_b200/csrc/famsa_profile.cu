@@ -316,3 +316,91 @@ extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off
     if (own_state) FAMSA_CUDA(cudaFreeAsync(own_state, st));
     return FAMSA_OK;
 }
+
+// ---- famsa_seqprof_scores_static: the score-only alignment batch for callers that must not allocate ----------
+// (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  The same seqprof_kernel<J>
+// instantiations as famsa_seqprof_align; what that call takes from cudaMallocAsync / cudaMallocHost -- the device copy
+// of the alignment descriptors and one final-state byte per alignment -- lives in a file-scope device array of fixed
+// size instead, and the host-side staging of the descriptors in a file-scope host array.  Every GPU that loads the
+// library holds the device array (FAMSA_SEQPROF_STATIC_MAX x 49 bytes = 0.8 MB) until the process exits.
+namespace famsa {
+
+constexpr size_t STATIC_DESC_BYTES = sizeof(AlignDesc) * (size_t)FAMSA_SEQPROF_STATIC_MAX;
+static __device__ __align__(256) unsigned char g_seqprof_scratch[STATIC_DESC_BYTES + (size_t)FAMSA_SEQPROF_STATIC_MAX];
+// In HOST code `g_seqprof_scratch` is only a stand-in for the symbol, not a device address: the address a kernel may
+// use comes from cudaGetSymbolAddress, taken once per device with that device current.
+constexpr int STATIC_MAX_DEVICES = 64;
+static std::mutex g_static_mu;                                    // guards the address table AND the host staging array
+static unsigned char* g_static_dev_ptr[STATIC_MAX_DEVICES] = {};
+static AlignDesc g_static_host_desc[FAMSA_SEQPROF_STATIC_MAX];    // host staging (static storage, pageable)
+
+}  // namespace famsa
+
+extern "C" int famsa_seqprof_scores_static(const float* cost_dev, const int64_t* col_off_host, const uint8_t* seq_dev,
+                                           const int64_t* seq_off_host, const float* gaps_dev, const int32_t* nseq_dev,
+                                           int64_t n_align, float* score_dev, void* cuda_stream) {
+    if (n_align > FAMSA_SEQPROF_STATIC_MAX) {
+        set_error("famsa_seqprof_scores_static: n_align exceeds FAMSA_SEQPROF_STATIC_MAX (16384 alignments per call): "
+                  "split the batch, or use famsa_seqprof_align");
+        return FAMSA_ERANGE;
+    }
+    int rc = seqprof_check(col_off_host, seq_off_host, n_align, "famsa_seqprof_scores_static");
+    if (rc != FAMSA_OK) return rc;
+    if (n_align == 0) return FAMSA_OK;
+    if (!cost_dev || !seq_dev || !gaps_dev || !nseq_dev || !score_dev) { set_error("famsa_seqprof_scores_static: null pointer"); return FAMSA_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int device = -1;
+    FAMSA_CUDA(cudaGetDevice(&device));
+    if (device < 0 || device >= STATIC_MAX_DEVICES) { set_error("famsa_seqprof_scores_static: device ordinal out of range"); return FAMSA_ECUDA; }
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_dev_ptr[device]) {                                 // set-up, once per device, that device being current
+        unsigned char* p = nullptr;
+        FAMSA_CUDA(cudaGetSymbolAddress((void**)&p, g_seqprof_scratch));
+        if (!p) { set_error("famsa_seqprof_scores_static: cudaGetSymbolAddress returned no address"); return FAMSA_ECUDA; }
+        g_static_dev_ptr[device] = p;
+    }
+    AlignDesc* d_desc = reinterpret_cast<AlignDesc*>(g_static_dev_ptr[device]);
+    uint8_t* final_state = g_static_dev_ptr[device] + STATIC_DESC_BYTES;
+    // descriptors grouped by residues per lane, heaviest group first: a counting sort over the 8 classes into the static
+    // host array (no heap allocation on this path)
+    int64_t start[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};                  // class c = 8 - J/4 (J = 32 first)
+    for (int64_t b = 0; b < n_align; ++b) start[8 - lanes_j(seq_off_host[b + 1] - seq_off_host[b]) / 4 + 1]++;
+    for (int c = 0; c < 8; ++c) start[c + 1] += start[c];
+    int64_t fill[8];
+    for (int c = 0; c < 8; ++c) fill[c] = start[c];
+    for (int64_t b = 0; b < n_align; ++b) {
+        const int j = lanes_j(seq_off_host[b + 1] - seq_off_host[b]);
+        AlignDesc& d = g_static_host_desc[fill[8 - j / 4]++];
+        d.cost_row0 = col_off_host[b]; d.seq0 = seq_off_host[b];
+        d.n1 = (int32_t)(col_off_host[b + 1] - col_off_host[b]); d.n2 = (int32_t)(seq_off_host[b + 1] - seq_off_host[b]);
+        d.idx = (int32_t)b; d.j = j;
+        d.dir0 = 0; d.path_end = 0;                                  // no traceback in this variant
+    }
+    // The array keeps the previous call's contents.  Nothing in it has to start at zero: every descriptor and every
+    // final-state byte a call reads is written by that call first; the final-state bytes are cleared all the same, so
+    // that no value of an earlier call can ever be mistaken for this one's.
+    FAMSA_CUDA(cudaMemsetAsync(final_state, 0, (size_t)n_align, st));
+    // pageable source: the runtime has staged the bytes when the call returns, so the host array is free again
+    FAMSA_CUDA(cudaMemcpyAsync(d_desc, g_static_host_desc, sizeof(AlignDesc) * (size_t)n_align, cudaMemcpyHostToDevice, st));
+    for (int c = 0; c < 8; ++c) {
+        const int64_t g0 = start[c];
+        const int n = (int)(start[c + 1] - start[c]);
+        if (n == 0) continue;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)((n + 3) / 4)); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = RING_BYTES; cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        cudaError_t le = cudaSuccess;
+#define SEQPROF_STATIC_CASE(JJ) case JJ: le = cudaLaunchKernelEx(&cfg, seqprof_kernel<JJ>, (const AlignDesc*)(d_desc + g0), n, cost_dev, seq_dev, \
+                                                                 gaps_dev, nseq_dev, score_dev, final_state, (uint8_t*)nullptr, 0); break;
+        switch (32 - 4 * c) {
+            SEQPROF_STATIC_CASE(4) SEQPROF_STATIC_CASE(8) SEQPROF_STATIC_CASE(12) SEQPROF_STATIC_CASE(16)
+            SEQPROF_STATIC_CASE(20) SEQPROF_STATIC_CASE(24) SEQPROF_STATIC_CASE(28) SEQPROF_STATIC_CASE(32)
+        }
+#undef SEQPROF_STATIC_CASE
+        FAMSA_CUDA(le);
+    }
+    return FAMSA_OK;
+}

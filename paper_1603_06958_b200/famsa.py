@@ -24,7 +24,9 @@ EXPORTS = ["famsa_pack", "famsa_lcs_rows", "famsa_lcs_rows_host", "famsa_lcs_row
            "famsa_tree_edges", "famsa_tree_finish", "famsa_tree_free",
            "famsa_guide_tree", "famsa_guide_forest"]
 # include/famsa_profile.h
-EXPORTS_PROFILE = ["famsa_profile_costs", "famsa_gap_scale", "famsa_seqprof_workspace", "famsa_seqprof_align"]
+EXPORTS_PROFILE = ["famsa_profile_costs", "famsa_gap_scale", "famsa_seqprof_workspace", "famsa_seqprof_align",
+                   "famsa_seqprof_scores_static"]
+FAMSA_SEQPROF_STATIC_MAX = 16384
 
 
 class FamsaError(RuntimeError):
@@ -117,6 +119,8 @@ def lib():
         L.famsa_seqprof_workspace.argtypes = [vp, vp, i64]
         L.famsa_seqprof_align.restype = i32
         L.famsa_seqprof_align.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp]
+        L.famsa_seqprof_scores_static.restype = i32
+        L.famsa_seqprof_scores_static.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp]
         L.famsa_strerror.restype = ctypes.c_char_p
         L.famsa_strerror.argtypes = [i32]
         L.famsa_last_error.restype = ctypes.c_char_p
@@ -456,3 +460,17 @@ def famsa_seqprof_align(cost, col_off, seq, seq_off, gaps, nseq, score, path=Non
         assert workspace.numel() >= famsa_seqprof_workspace(col_off, seq_off)
     _check(lib().famsa_seqprof_align(_ptr(cost), col_off.ctypes.data, _ptr(seq), seq_off.ctypes.data, _ptr(gaps), _ptr(nseq), B,
                                      _ptr(score), _ptr(path), _ptr(path_len), _ptr(workspace), _stream(cuda_stream)))
+
+
+def famsa_seqprof_scores_static(cost, col_off, seq, seq_off, gaps, nseq, score, cuda_stream=None):
+    """Score-only famsa_seqprof_align that allocates nothing (scratch in a static device array; at most
+    FAMSA_SEQPROF_STATIC_MAX alignments per call; overlapping calls on one GPU race: see include/famsa_profile.h)."""
+    col_off = np.ascontiguousarray(col_off, dtype=np.int64)
+    seq_off = np.ascontiguousarray(seq_off, dtype=np.int64)
+    B = col_off.size - 1
+    assert seq_off.size == B + 1
+    for t, size in ((cost, 4), (seq, 1), (gaps, 4), (nseq, 4), (score, 4)):
+        assert t.is_cuda and t.is_contiguous() and t.element_size() == size
+    assert gaps.numel() >= 4 * B and nseq.numel() >= B and score.numel() >= B
+    _check(lib().famsa_seqprof_scores_static(_ptr(cost), col_off.ctypes.data, _ptr(seq), seq_off.ctypes.data, _ptr(gaps), _ptr(nseq), B,
+                                             _ptr(score), _stream(cuda_stream)))
