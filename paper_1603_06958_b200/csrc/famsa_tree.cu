@@ -574,8 +574,11 @@ __global__ void __launch_bounds__(DG_B) tree_dendrogram_kernel(uint32_t k, const
     __shared__ uint16_t s_par[2 * DG_B];                   // local union-find over canonical slots
     __shared__ uint16_t s_hidx[2 * DG_B];
     __shared__ uint2 s_info[2 * DG_B];                     // (.x = size, .y = cluster id) of a local root
-    __shared__ uint32_t s_oa[DG_B], s_ob[DG_B], s_os[DG_B];
-    __shared__ uint32_t h_key[DG_H], h_slot[DG_H];
+    __shared__ uint32_t h_key[DG_H], h_slot[DG_H];          // hash table of phase B; afterwards reused:
+    uint32_t* const s_cnt = h_key;                          //   [2 DG_B] references to each canonical slot in this batch
+    uint32_t* const s_oa = h_slot; uint32_t* const s_ob = h_slot + DG_B; uint32_t* const s_os = h_slot + 2 * DG_B;   // merge outputs
+    uint16_t* const s_hub = s_hidx;                         //   [DG_B] the edge's hub slot (0xFFFF: none)
+    static_assert(2 * DG_B <= DG_H && 3 * DG_B <= DG_H, "aliases fit");
     const uint32_t tid = threadIdx.x, m = k - 1;
     uint32_t nx = 0, ny = 0; float nw = 0.0f;              // this thread's edge of the next batch
     if (tid < m) { const uint32_t e = order[tid]; nx = ta[e]; ny = tb[e]; nw = tw[e]; }
@@ -610,15 +613,68 @@ __global__ void __launch_bounds__(DG_B) tree_dendrogram_kernel(uint32_t k, const
             s_par[s] = (uint16_t)s;
         }
         __syncthreads();
-        for (uint32_t s = tid; s < 2 * nb; s += DG_B) {
+        uint32_t my_c[2];                                   // (2 slots per thread: 2 nb <= 2 DG_B)
+        for (uint32_t s = tid, n = 0; s < 2 * nb; s += DG_B, ++n) {
             const uint32_t c = h_slot[s_hidx[s]];
-            s_canon[s] = (uint16_t)c;
+            my_c[n] = c;
             if (c == s) { const unsigned long long v = __ldcg(info + s_root[s]); s_info[s] = make_uint2((uint32_t)v, (uint32_t)(v >> 32)); }
         }
+        __syncthreads();                                    // the hash table is free from here on
+        for (uint32_t s = tid, n = 0; s < 2 * nb; s += DG_B, ++n) { s_canon[s] = (uint16_t)my_c[n]; s_cnt[s] = 0; }
         __syncthreads();
+        for (uint32_t s = tid; s < 2 * nb; s += DG_B) atomicAdd(&s_cnt[s_canon[s]], 1u);
+        __syncthreads();
+        // Classification.  A canonical slot referenced more than once in the batch is a HUB (in single linkage: the growing
+        // cluster that the next edges chain onto).  If no edge joins two hubs, the batch falls apart into independent
+        // pieces -- free edges (both sets referenced once) and one chain per hub, whose k-th edge only needs the running
+        // (id, size) of its hub -- and phase C runs in parallel; otherwise one thread does the batch's unions in order.
+        bool bad = false;
+        if (tid < nb) {
+            const uint32_t cx = s_canon[2 * tid], cy = s_canon[2 * tid + 1];
+            const bool hx = s_cnt[cx] > 1, hy = s_cnt[cy] > 1;
+            bad = (hx && hy) || cx == cy;
+            s_hub[tid] = (uint16_t)(hx ? cx : (hy ? cy : 0xFFFFu));
+        }
+        const bool serial = __syncthreads_or(bad);
         // C: the unions, in edge order.  One thread, so what counts is the length of its dependent instruction
         // chain per edge: 32-bit (id, size) halves, results to shared memory (phase D writes them out, widened).
-        if (tid == 0) {
+        if (!serial) {
+            const uint32_t id0 = k + t0;
+            if (tid < nb && s_hub[tid] == 0xFFFFu) {        // a free edge: nothing else in the batch touches its two sets
+                const uint32_t x = s_canon[2 * tid], y = s_canon[2 * tid + 1];
+                const uint2 ix = s_info[x], iy = s_info[y];
+                const uint32_t sz = ix.x + iy.x;
+                s_oa[tid] = min(ix.y, iy.y); s_ob[tid] = max(ix.y, iy.y); s_os[tid] = sz;
+                const bool keep_x = ix.x >= iy.x;
+                s_par[keep_x ? y : x] = (uint16_t)(keep_x ? x : y);
+                s_info[keep_x ? x : y] = make_uint2(sz, id0 + tid);
+            }
+            for (uint32_t h = tid; h < 2 * nb; h += DG_B) { // one thread per hub walks the hub's edges in order
+                if (s_canon[h] != h || s_cnt[h] < 2) continue;
+                uint2 run = s_info[h];                      // the hub's running (size, id)
+                for (uint32_t q0 = 0; q0 < nb; q0 += 4) {   // four edges at a time: their loads do not depend on `run`
+                    uint32_t hub[4], oth[4]; uint2 io[4];
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        const uint32_t q = min(q0 + r, nb - 1);
+                        hub[r] = q0 + r < nb ? s_hub[q] : 0xFFFFu;
+                        const uint32_t c0 = s_canon[2 * q], c1 = s_canon[2 * q + 1];
+                        oth[r] = c0 == h ? c1 : c0;
+                    }
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) io[r] = s_info[oth[r]];
+#pragma unroll
+                    for (int r = 0; r < 4; ++r)
+                        if (hub[r] == h) {
+                            const uint32_t q = q0 + r, sz = run.x + io[r].x;
+                            s_oa[q] = min(run.y, io[r].y); s_ob[q] = max(run.y, io[r].y); s_os[q] = sz;
+                            s_par[oth[r]] = (uint16_t)h;
+                            run = make_uint2(sz, id0 + q);
+                        }
+                }
+                s_info[h] = run;
+            }
+        } else if (tid == 0) {
             const uint32_t* canon2 = reinterpret_cast<const uint32_t*>(s_canon);
             uint32_t cc = canon2[0];
             const uint32_t id0 = k + t0;
