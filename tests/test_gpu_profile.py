@@ -76,10 +76,11 @@ def test_batch_against_oracle(F):
 
 
 def test_every_lane_width_and_the_edges(F):
-    """n2 at both sides of every residues-per-lane boundary (multiples of 128 up to 1024), the smallest inputs, long and short profiles."""
+    """n2 at both sides of every residues-per-lane boundary (multiples of 64 up to 1024), the smallest inputs, long and short profiles."""
     from paper_1603_06958_b200 import synth
     subst = synth.substitution_matrix()
-    lengths = [(1, 1), (1, 5), (7, 1), (2, 2), (40, 127), (40, 128), (40, 129), (33, 256), (33, 257), (35, 384), (35, 385), (90, 511),
+    lengths = [(1, 1), (1, 5), (7, 1), (2, 2), (20, 63), (20, 64), (20, 65), (25, 191), (25, 192), (25, 193), (30, 320), (30, 321), (30, 448),
+               (30, 449), (30, 576), (30, 577), (30, 704), (30, 705), (30, 832), (30, 833), (30, 960), (30, 961), (40, 127), (40, 128), (40, 129), (33, 256), (33, 257), (35, 384), (35, 385), (90, 511),
                (90, 512), (90, 513), (50, 640), (50, 641), (45, 768), (45, 769), (45, 896), (45, 897), (60, 1023), (60, 1024),
                (1500, 31), (900, 300), (5, 700), (31, 32), (32, 33), (64, 4)]
     counts, col_off, seq, seq_off, nseq = synth.profile_batch(len(lengths), seed=402, lengths=lengths)
