@@ -562,9 +562,11 @@ def run_cuda(args, rank, world, local_rank):
     peak1 = F.famsa_alu_peak(local_rank)
     mix1 = F.famsa_mix_peak(local_rank)
     ctx.free()
+    if dist is not None:                  # every collective is behind us: leave the group together, BEFORE rank 0's
+        dist.barrier()                    # CPU legs (tens of seconds), so that no rank tears down a communicator
+        dist.destroy_process_group()      # whose peers have already exited
+        dist = None
     if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
         return
 
     # ---- rank 0: the oracle beside it (and against it), the roofline, the line
