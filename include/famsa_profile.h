@@ -62,7 +62,7 @@ int64_t famsa_seqprof_workspace(const int64_t* col_off_host, const int64_t* seq_
  *                 first, RIGHT-ALIGNED in the segment [col_off[b] + seq_off[b], col_off[b+1] + seq_off[b+1]) (its
  *                 capacity n1 + n2): they start at segment_end - path_len[b]
  *   path_len_dev  DEVICE int32 [n_align] (required with path_dev)
- *   workspace_dev DEVICE, famsa_seqprof_workspace bytes (may be NULL when path_dev is NULL)
+ *   workspace_dev DEVICE, famsa_seqprof_workspace bytes, 16-byte aligned (may be NULL when path_dev is NULL)
  * Enqueued on cuda_stream; the offset arrays are copied before the call returns.
  * Errors: FAMSA_EINVAL (null pointers, offsets), FAMSA_ELENGTH (an empty or too long sequence, an empty profile),
  * FAMSA_ENOMEM, FAMSA_ECUDA.

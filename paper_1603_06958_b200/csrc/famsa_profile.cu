@@ -12,7 +12,7 @@
 // direction byte (2 bits per state).  All arithmetic is fp32 adds,
 // subtractions and comparisons in the order the oracle's fp32 mode uses (products of nseq and a gap cost are
 // formed once with __fmul_rn, nothing can contract into an FMA), so scores AND traceback decisions are
-// bit-identical to it.  A second kernel (one thread per alignment) walks the direction bytes back.
+// bit-identical to it.  A second kernel (one warp per alignment, tile by tile) walks the direction bytes back.
 // (Tried, r02: loading the lane's cost values one row ahead -- +16 registers at J = 16 -- was 1 % slower.)
 // (Tried, r02: J in steps of 2 instead of 4 -- half the idle lane slots, but 16-bit direction stores for J = 2 mod 4
 //  and twice as many, smaller launches: 245 against 262 GCUPS at 8192 alignments, 304 against 320 at 32768.)
@@ -162,29 +162,67 @@ __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restric
     asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
-// One thread per alignment walks the direction bytes from (n1, n2) back to (0, 0); the operations are written
-// right-aligned into the alignment's path segment.
-__global__ void seqprof_trace_kernel(const AlignDesc* __restrict__ desc, int n, const uint8_t* __restrict__ final_state,
-                                     const uint8_t* __restrict__ ws, uint8_t* __restrict__ path, int32_t* __restrict__ path_len) {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= n) return;
-    const AlignDesc d = desc[t];
+// Traceback: one WARP per alignment walks the direction bytes from (n1, n2) back to (0, 0); the operations are written
+// right-aligned into the alignment's path segment.  The walk itself is a dependent chain (one thread), but its memory
+// latency is not: the warp first loads the 32 x 32-cell tile of direction bytes whose lower right corner is the current
+// cell (lane l: DP row i - l, eight aligned 32-bit words; a word never straddles a lane block of the skewed layout
+// because J is a multiple of 4), lane 0 then walks inside the tile out of shared memory (at least 32, at most 63 steps),
+// and the warp writes that stretch of the path out together.  One thread per alignment with a global load per step took
+// 0.65 ms for 8192 alignments (long scoreboard: 19 warps per issue); see DESIGN.md 6.8 for the number now.
+constexpr int TRACE_T = 32;
+__global__ void __launch_bounds__(128) seqprof_trace_kernel(const AlignDesc* __restrict__ desc, int n, const uint8_t* __restrict__ final_state,
+                                                            const uint8_t* __restrict__ ws, uint8_t* __restrict__ path, int32_t* __restrict__ path_len) {
+    __shared__ uint32_t tile_all[4][TRACE_T][TRACE_T / 4 + 1];
+    __shared__ uint8_t ops_all[4][2 * TRACE_T];
+    const int warp = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+    if (warp >= n) return;
+    uint32_t (*tile)[TRACE_T / 4 + 1] = tile_all[threadIdx.x >> 5];
+    uint8_t* ops = ops_all[threadIdx.x >> 5];
+    const AlignDesc d = desc[warp];
     const uint8_t* dir = ws + d.dir0;
-    const int stride = 32 * d.j;
+    const int stride = 32 * d.j, J = d.j;
     int i = d.n1, j = d.n2, len = 0;
     uint32_t st = final_state[d.idx];
-    uint8_t* out = path + d.path_end;
-    while (i > 0 || j > 0) {
-        uint32_t dd;
-        if (i > 0 && j > 0) dd = dir[(size_t)(i - 1 + (j - 1) / d.j) * stride + (j - 1)];   // skewed rows: see seqprof_kernel
-        else if (i == 0) dd = (j == 1 ? 0u : 2u) << 4;        // row 0: a run of terminal gap columns
-        else dd = (i == 1 ? 0u : 1u) << 2;                    // residue 0: a run of terminal gaps
-        *--out = (uint8_t)st; ++len;
-        if (st == 0) { st = dd & 3; --i; --j; }
-        else if (st == 1) { st = (dd >> 2) & 3; --i; }
-        else { st = (dd >> 4) & 3; --j; }
+    uint8_t* out = path + d.path_end;                        // one past the next operation's place (the path is written backwards)
+    while (i > 0 && j > 0) {                                 // warp-uniform: i, j, st are broadcast after every tile
+        const int hi = ((j - 1) | 3) + 1, lo = max(0, hi - TRACE_T);      // zero-based columns [lo, hi), both multiples of 4
+        const int ri = i - lane;                             // this lane's DP row
+#pragma unroll
+        for (int w = 0; w < TRACE_T / 4; ++w) {
+            const int cz = lo + 4 * w;
+            uint32_t v = 0;
+            if (ri >= 1 && cz < hi) v = __ldg(reinterpret_cast<const uint32_t*>(dir + (size_t)(ri - 1 + cz / J) * stride + cz));
+            tile[lane][w] = v;
+        }
+        __syncwarp();
+        int steps = 0;
+        if (lane == 0) {
+            const int i_top = i;
+            while (i > 0 && j > 0 && i_top - i < TRACE_T && j - 1 >= lo) {
+                const uint32_t dd = (tile[i_top - i][(j - 1 - lo) >> 2] >> (8 * ((j - 1) & 3))) & 0xFFu;
+                ops[steps++] = (uint8_t)st;
+                if (st == 0) { st = dd & 3; --i; --j; }
+                else if (st == 1) { st = (dd >> 2) & 3; --i; }
+                else { st = (dd >> 4) & 3; --j; }
+            }
+        }
+        __syncwarp();
+        i = __shfl_sync(0xffffffffu, i, 0); j = __shfl_sync(0xffffffffu, j, 0);
+        st = __shfl_sync(0xffffffffu, st, 0); steps = __shfl_sync(0xffffffffu, steps, 0);
+        for (int q = lane; q < steps; q += 32) out[-1 - q] = ops[q];
+        out -= steps; len += steps;
+        __syncwarp();
     }
-    path_len[d.idx] = len;
+    if (lane == 0) {
+        while (i > 0 || j > 0) {                             // along a border: runs of terminal gaps, no memory involved
+            const uint32_t dd = i == 0 ? (j == 1 ? 0u : 2u) << 4 : (i == 1 ? 0u : 1u) << 2;
+            *--out = (uint8_t)st; ++len;
+            if (st == 0) { st = dd & 3; --i; --j; }
+            else if (st == 1) { st = (dd >> 2) & 3; --i; }
+            else { st = (dd >> 4) & 3; --j; }
+        }
+        path_len[d.idx] = len;
+    }
 }
 
 // residues per lane: the smallest multiple of 4 with 32 J >= n2 (4 .. 32), so at most 127 of the 32 J lane slots idle
@@ -244,6 +282,7 @@ extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off
     if (!cost_dev || !seq_dev || !gaps_dev || !nseq_dev || !score_dev || (path_dev && (!path_len_dev || !workspace_dev))) {
         set_error("famsa_seqprof_align: null pointer (path_dev needs path_len_dev and workspace_dev)"); return FAMSA_EINVAL;
     }
+    if (reinterpret_cast<uintptr_t>(workspace_dev) & 15) { set_error("famsa_seqprof_align: workspace_dev must be 16-byte aligned"); return FAMSA_EINVAL; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     // descriptors, grouped by residues-per-lane variant (longest profiles first inside a group: the heavy warps start first)
     std::vector<AlignDesc> desc((size_t)n_align);
@@ -312,7 +351,7 @@ extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off
         g0 = g1;
     }
     if (path_dev)
-        seqprof_trace_kernel<<<(unsigned)((n_align + 127) / 128), 128, 0, st>>>(d_desc, (int)n_align, final_state, ws, path_dev, path_len_dev);
+        seqprof_trace_kernel<<<(unsigned)((n_align + 3) / 4), 128, 0, st>>>(d_desc, (int)n_align, final_state, ws, path_dev, path_len_dev);
     FAMSA_CUDA(cudaGetLastError());
     FAMSA_CUDA(cudaFreeAsync(d_desc, st));
     if (own_state) FAMSA_CUDA(cudaFreeAsync(own_state, st));
