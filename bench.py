@@ -66,6 +66,10 @@ def parse_args():
     ap.add_argument("--workload", default="lcs", choices=["lcs", "seqprof"],
                     help="lcs: the all-pairs LCS sweep (the headline, default); seqprof: SURVEY 8(f) NEXT-4, a batch of sequence-vs-profile alignments")
     ap.add_argument("--batch", type=int, default=8192, help="alignments per step of --workload seqprof")
+    ap.add_argument("--rehearse-one-gpu", action="store_true",
+                    help="REHEARSAL of the N > 1 host logic on a box with one GPU: every rank uses cuda:0 and the process group is "
+                         "gloo (NCCL refuses two ranks on one device).  The ranks time-slice the GPU, so the numbers mean nothing; "
+                         "what it shows is that dealing, reductions, forest gather + merge and the teardown run end to end")
     ap.add_argument("--kernel-only", action="store_true",
                     help="profiling runs: only the device-resident timed steps (no e2e, full-sweep, guide-tree or CPU legs)")
     ap.add_argument("--host-mode", type=int, default=-1, choices=[-1, 0, 1],
@@ -338,9 +342,14 @@ def run_cuda(args, rank, world, local_rank):
     dist = None
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if args.rehearse_one_gpu:
+            local_rank = 0
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
+    coll_dev = torch.device("cpu") if args.rehearse_one_gpu else dev     # where the tensors of the collectives live
 
     seqs, offsets = synth.family(args.config, k=args.k)      # replicated on every rank
     k = len(offsets) - 1
@@ -409,7 +418,7 @@ def run_cuda(args, rank, world, local_rank):
     ms_total = ev[0].elapsed_time(ev[-1])
     step_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)] if per_step_events else None
     ms_rank = ms_total
-    ms_total, cells_all, pairs_all = reduce_over_ranks(dist, ms_total, cells_step, pairs_step, dev)
+    ms_total, cells_all, pairs_all = reduce_over_ranks(dist, ms_total, cells_step, pairs_step, coll_dev)
     sec = ms_total * 1e-3
     value = cells_all * args.steps / sec / 1e9
     ck_timed = ck.cpu().numpy().astype(np.uint64)
@@ -487,7 +496,7 @@ def run_cuda(args, rank, world, local_rank):
     barrier()
     e2e_sec = max(time.perf_counter() - t0, 1e-9)
     if dist is not None:
-        t = torch.tensor([e2e_sec], dtype=torch.float64, device=dev)
+        t = torch.tensor([e2e_sec], dtype=torch.float64, device=coll_dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_sec = float(t.item())
     e2e_value = cells_all * e2e_steps / e2e_sec / 1e9
@@ -535,7 +544,7 @@ def run_cuda(args, rank, world, local_rank):
         forest = F.famsa_guide_forest(ctx, BLOCK_ROWS, rank, world)
         t_forest = time.perf_counter() - t0
         fa, fb, fw = F.famsa_tree_edges(forest)
-        parts = gather_forests(dist, fa, fb, fw, k, dev)
+        parts = gather_forests(dist, fa, fb, fw, k, coll_dev)
         n_merges = 0
         t1 = time.perf_counter()
         if rank == 0:
@@ -548,7 +557,7 @@ def run_cuda(args, rank, world, local_rank):
         dt = time.perf_counter() - t0
         forest.free()
         if dist is not None:
-            tt = torch.tensor([dt], dtype=torch.float64, device=dev)
+            tt = torch.tensor([dt], dtype=torch.float64, device=coll_dev)
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
             dt = float(tt.item())
         fcells = F.famsa_rows_cells(ctx, 0, k)
