@@ -687,9 +687,14 @@ def run_seqprof(args, rank, world, local_rank):
     dist = None
     if world > 1:                      # alignments are independent: every rank takes its own batch, no collective
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if args.rehearse_one_gpu:
+            local_rank = 0
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
+    coll_dev = torch.device("cpu") if args.rehearse_one_gpu else dev
     B = args.batch
     counts, col_off, seq, seq_off, nseq = synth.profile_batch(B, seed=SEQPROF_SEED + rank, n1_range=(100, 700))
     subst = synth.substitution_matrix()
@@ -725,7 +730,7 @@ def run_seqprof(args, rank, world, local_rank):
     torch.cuda.synchronize()
     clocks = sampler.stop()
     ms_rank = e0.elapsed_time(e1)
-    ms, cells_all, _ = reduce_over_ranks(dist, ms_rank, cells, B, dev)      # max time over ranks, sum of the cells
+    ms, cells_all, _ = reduce_over_ranks(dist, ms_rank, cells, B, coll_dev)      # max time over ranks, sum of the cells
     value = cells_all * args.steps / ms / 1e6
     peak = F.famsa_alu_peak(local_rank)
     # Roofline: the ALU pipe.  Per cell and state: 2 compares + 2 value selects + 2 direction selects on
@@ -750,7 +755,7 @@ def run_seqprof(args, rank, world, local_rank):
         e2e_step()
     e2e_sec = time.perf_counter() - t0
     if dist is not None:
-        tt = torch.tensor([e2e_sec], dtype=torch.float64, device=dev)
+        tt = torch.tensor([e2e_sec], dtype=torch.float64, device=coll_dev)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         e2e_sec = float(tt.item())
         dist.destroy_process_group()
