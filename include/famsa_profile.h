@@ -47,8 +47,9 @@ int64_t famsa_seqprof_workspace(const int64_t* col_off_host, const int64_t* seq_
 
 /*
  * famsa_seqprof_align -- a batch of n_align INDEPENDENT alignments ("profile alignments in the bottom part of the
- * guide tree are independent, they can be performed in parallel").  One warp per alignment: lane l
- * owns J = 4 ceil(n2/128) consecutive residues with its three previous-row values per residue in registers and
+ * guide tree are independent, they can be performed in parallel").  One warp per alignment (16 lanes per
+ * alignment, two alignments per warp, when n2 <= 256): lane l
+ * owns J = 4 ceil(n2/128) (4 ceil(n2/64) with 16 lanes) consecutive residues with its three previous-row values per residue in registers and
  * sweeps the profile columns in a skewed wavefront (lane l works on column t - l at step t; the boundary values
  * move right by one shuffle per step); one direction byte per cell goes to the workspace and a second kernel
  * walks it back.

@@ -2,8 +2,8 @@
 // (PAPER.md:71-79, 107, 111-116, 133-139).  Boundary and the readings of the paper: include/famsa_profile.h,
 // DESIGN.md P1-P9.
 //
-// Mapping: one warp per alignment.  The SEQUENCE side (n2 <= 1024 residues) is spread over the 32 lanes, J =
-// 4, 8, ... 32 consecutive residues per lane, and for each of them the lane keeps the three states of the
+// Mapping: one warp per alignment (two alignments per warp, 16 lanes each, for sequences of <= 256 residues).  The
+// SEQUENCE side (n2 <= 1024 residues) is spread over the lanes, J = 4, 8, ... 32 consecutive residues per lane, and for each of them the lane keeps the three states of the
 // previous profile column (row) in registers: 3 J floats.  The rows are swept in a skewed wavefront: at step t
 // lane l computes row t - l + 1, so what it needs from the left -- the three states of lane l-1's last residue
 // in the same row -- was produced one step earlier and arrives by one __shfl_up per state; the value received
@@ -27,15 +27,20 @@
 namespace famsa {
 
 constexpr float NEG = -3.0e38f;
-constexpr int RING_ROWS = 64, RING_STRIDE = 33;              // per-warp ring of cost rows in shared memory (floats)
-constexpr size_t RING_BYTES = 4 * RING_ROWS * RING_STRIDE * sizeof(float);   // 4 warps per CTA
+constexpr int RING_STRIDE = 33;                              // per-alignment ring of cost rows in shared memory: 2 SEG rows of 33 floats
+constexpr size_t RING_BYTES = 4 * 64 * RING_STRIDE * sizeof(float);   // 4 warps per CTA x (32 / SEG) alignments x 2 SEG rows
+#ifndef SEQPROF_SEG16_MAX
+#define SEQPROF_SEG16_MAX 256                                // sequences up to this length take 16 lanes (two alignments per warp);
+                                                             // measured r02: 256 -> +7-8 % on batches of short sequences, 512 -> -20 % (J >= 20: 255 registers)
+#endif
 
 struct AlignDesc {
     int64_t cost_row0;       // first cost row of the profile
     int64_t seq0;            // first residue of the sequence
-    int64_t dir0;            // byte offset of the direction bytes in the workspace (n1 + 31 skewed rows of 32 J bytes)
+    int64_t dir0;            // byte offset of the direction bytes in the workspace (n1 + seg - 1 skewed rows of seg x J bytes)
     int64_t path_end;        // end of the path segment
-    int32_t n1, n2, idx, j;  // columns, residues, index in the batch, residues per lane
+    int32_t n1, n2, idx;     // columns, residues, index in the batch
+    int16_t j, seg;          // residues per lane, lanes per alignment (32, or 16: two alignments share a warp)
 };
 
 __global__ void profile_costs_kernel(const uint32_t* __restrict__ counts, const float* __restrict__ subst, int64_t n_cols, float* __restrict__ cost) {
@@ -48,7 +53,7 @@ __global__ void profile_costs_kernel(const uint32_t* __restrict__ counts, const 
     cost[t] = (float)s;
 }
 
-template <int J>
+template <int J, int SEG>
 __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restrict__ desc, int n, const float* __restrict__ cost,
                                                       const uint8_t* __restrict__ seq, const float* __restrict__ gaps,
                                                       const int32_t* __restrict__ nseq, float* __restrict__ score,
@@ -59,14 +64,21 @@ __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restric
     // griddepcontrol.wait, so a group cannot complete before its predecessor and the traceback kernel -- an
     // ordinary launch after the last group -- sees all of them.
     asm volatile("griddepcontrol.launch_dependents;");
+    // SEG lanes per alignment: 32 (one alignment per warp) or 16 (two: short sequences would leave lanes idle and pay the
+    // full 31-step skew; with 16 lanes the same registers hold twice the residues per lane, which also gives each lane
+    // more independent work per step).  An idle second segment runs with n1 = 0: it takes part in the warp's shuffles
+    // and barriers and never computes or stores.
+    constexpr int APW = 32 / SEG, RROWS = 2 * SEG;
     const int warp = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
-    if (warp >= n) return;
-    const AlignDesc d = desc[warp];
-    const int n1 = d.n1, n2 = d.n2, b = d.idx;
+    const int sl = lane & (SEG - 1), seg = lane / SEG;
+    if (warp * APW >= n) return;
+    const bool valid = warp * APW + seg < n;
+    const AlignDesc d = desc[valid ? warp * APW + seg : n - 1];
+    const int n1 = valid ? d.n1 : 0, n2 = d.n2, b = d.idx;
     const float To = gaps[4 * b], Te = gaps[4 * b + 1], Go = gaps[4 * b + 2], Ge = gaps[4 * b + 3];
     const float ns = (float)nseq[b];
     const float nTo = __fmul_rn(ns, To), nTe = __fmul_rn(ns, Te), nGo = __fmul_rn(ns, Go), nGe = __fmul_rn(ns, Ge);
-    const int j0 = lane * J;                                 // this lane owns residues j0+1 .. j0+J (1-based)
+    const int j0 = sl * J;                                   // this lane owns residues j0+1 .. j0+J (1-based)
     uint32_t yw[J / 4];                                      // their codes, 4 per word (code*4 = byte offset in a cost row)
 #pragma unroll
     for (int q = 0; q < J / 4; ++q) {
@@ -78,7 +90,7 @@ __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restric
     // row 0: residues before the first column are terminal gap columns, Y[0][j] = Y[0][j-1] - nseq T_e
     float yrun = 0.0f;
     for (int j = 1; j <= j0; ++j) yrun = j == 1 ? 0.0f - nTo : yrun - nTe;
-    float dM = lane == 0 ? 0.0f : NEG, dX = NEG, dY = lane == 0 ? NEG : yrun;     // row 0 at residue j0: the first diagonal
+    float dM = sl == 0 ? 0.0f : NEG, dX = NEG, dY = sl == 0 ? NEG : yrun;         // row 0 at residue j0: the first diagonal
     float Mp[J], Xp[J], Yp[J];
 #pragma unroll
     for (int c = 0; c < J; ++c) { yrun = (j0 + c + 1) == 1 ? 0.0f - nTo : yrun - nTe; Mp[c] = NEG; Xp[c] = NEG; Yp[c] = yrun; }
@@ -92,20 +104,24 @@ __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restric
     // values from the ring; rows are 33 words apart, so the bank of (row r, symbol c) is (r + c) mod 32 and lanes on
     // different rows with the same residue do not collide systematically.
     extern __shared__ float ring_all[];
-    float* ring = ring_all + (threadIdx.x >> 5) * (RING_ROWS * RING_STRIDE);
-    ring[lane] = crow[lane];                                 // row 0 (n1 >= 1)
+    float* ring = ring_all + ((threadIdx.x >> 5) * APW + seg) * (RROWS * RING_STRIDE);
+#pragma unroll
+    for (int q = 0; q < APW; ++q) ring[sl + q * SEG] = crow[sl + q * SEG];      // row 0 (every profile has one)
     __syncwarp();
     uint8_t* dir = ws + d.dir0;
-    const int stride = 32 * J;
-    const int steps = n1 + 31;
+    const int stride = SEG * J;
+    int steps = n1 + SEG - 1;
+    if (APW > 1) steps = max(steps, __shfl_xor_sync(0xffffffffu, steps, SEG));   // warp-uniform: the longer of the two profiles
     for (int t = 0; t < steps; ++t) {
-        const int i = t - lane + 1;
-        const float next_row = t + 1 < n1 ? __ldg(crow + (size_t)(t + 1) * SYMS + lane) : 0.0f;   // cost row t+1, used from the next step on
-        float lM = __shfl_up_sync(0xffffffffu, rM, 1), lX = __shfl_up_sync(0xffffffffu, rX, 1), lY = __shfl_up_sync(0xffffffffu, rY, 1);
+        const int i = t - sl + 1;
+        float next_row[APW];                                 // cost row t+1, used from the next step on
+#pragma unroll
+        for (int q = 0; q < APW; ++q) next_row[q] = t + 1 < n1 ? __ldg(crow + (size_t)(t + 1) * SYMS + sl + q * SEG) : 0.0f;
+        float lM = __shfl_up_sync(0xffffffffu, rM, 1, SEG), lX = __shfl_up_sync(0xffffffffu, rX, 1, SEG), lY = __shfl_up_sync(0xffffffffu, rY, 1, SEG);
         if (i >= 1 && i <= n1) {
-        if (lane == 0) { x0 = i == 1 ? 0.0f - To : x0 - Te; lM = NEG; lX = x0; lY = NEG; }
+        if (sl == 0) { x0 = i == 1 ? 0.0f - To : x0 - Te; lM = NEG; lX = x0; lY = NEG; }
         const float goy = i == n1 ? nTo : nGo, gey = i == n1 ? nTe : nGe;
-        const float* ci = ring + ((i - 1) & (RING_ROWS - 1)) * RING_STRIDE;
+        const float* ci = ring + ((i - 1) & (RROWS - 1)) * RING_STRIDE;
         float cM = dM, cX = dX, cY = dY;                     // diagonal of the lane's first residue
         dM = lM; dX = lX; dY = lY;                           // ... and the next row's
         uint32_t dw[J / 4];
@@ -141,7 +157,7 @@ __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restric
         }
         rM = lM; rX = lX; rY = lY;
         // Direction bytes in a SKEWED layout: the bytes of (row i, lane l) go to workspace row t = i - 1 + l, so that
-        // at one step all lanes write into the same 32 J-byte row (coalesced) instead of into 32 different rows.
+        // at one step all lanes of the alignment write into the same SEG x J-byte row (coalesced) instead of SEG different rows.
         if (want_dir) {
             uint8_t* out = dir + (size_t)t * stride + j0;
             if (J % 16 == 0) {
@@ -156,7 +172,9 @@ __global__ void __launch_bounds__(128) seqprof_kernel(const AlignDesc* __restric
             }
         }
         }
-        ring[((t + 1) & (RING_ROWS - 1)) * RING_STRIDE + lane] = next_row;     // the slot's old row (t - 63) was last read at step t - 32
+#pragma unroll
+        for (int q = 0; q < APW; ++q)                        // the slot's old row (t + 1 - 2 SEG) was last read at step t - SEG
+            ring[((t + 1) & (RROWS - 1)) * RING_STRIDE + sl + q * SEG] = next_row[q];
         __syncwarp();
     }
     asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -180,7 +198,7 @@ __global__ void __launch_bounds__(128) seqprof_trace_kernel(const AlignDesc* __r
     uint8_t* ops = ops_all[threadIdx.x >> 5];
     const AlignDesc d = desc[warp];
     const uint8_t* dir = ws + d.dir0;
-    const int stride = 32 * d.j, J = d.j;
+    const int stride = d.seg * d.j, J = d.j;
     int i = d.n1, j = d.n2, len = 0;
     uint32_t st = final_state[d.idx];
     uint8_t* out = path + d.path_end;                        // one past the next operation's place (the path is written backwards)
@@ -234,7 +252,36 @@ static std::mutex g_desc_mu;
 static DescStage g_desc[2];
 static int g_desc_next = 0;
 
-static int lanes_j(int64_t n2) { return (int)(4 * ((n2 + 127) / 128)); }
+// lanes per alignment and residues per lane (a multiple of 4 with seg x J >= n2)
+struct Shape { int seg, j; };
+static Shape shape_of(int64_t n2) {
+    if (n2 <= SEQPROF_SEG16_MAX) return Shape{16, (int)(4 * ((n2 + 63) / 64))};
+    return Shape{32, (int)(4 * ((n2 + 127) / 128))};
+}
+static int64_t dir_bytes_of(int64_t n1, Shape sh) { return (n1 + sh.seg - 1) * sh.seg * sh.j; }
+static int shape_class(Shape sh) { return (sh.seg == 32 ? 0 : 8) + 8 - sh.j / 4; }     // 16 classes; within a seg: heaviest J first
+
+// One (seg, J) group of a batch: n alignments whose descriptors are consecutive.  Launched as a programmatic dependent of
+// whatever precedes it in the stream (see seqprof_kernel).
+static cudaError_t launch_seqprof_group(int seg, int j, const AlignDesc* d_desc, int n, const float* cost_dev, const uint8_t* seq_dev,
+                                        const float* gaps_dev, const int32_t* nseq_dev, float* score_dev, uint8_t* final_state,
+                                        uint8_t* ws, int want_dir, cudaStream_t st) {
+    const int per_cta = 4 * (32 / seg);                      // 4 warps x alignments per warp
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)((n + per_cta - 1) / per_cta)); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = RING_BYTES; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+#define SEQPROF_CASE(JJ) case JJ: return seg == 32 \
+        ? cudaLaunchKernelEx(&cfg, seqprof_kernel<JJ, 32>, d_desc, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir) \
+        : cudaLaunchKernelEx(&cfg, seqprof_kernel<JJ, 16>, d_desc, n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev, final_state, ws, want_dir);
+    switch (j) {
+        SEQPROF_CASE(4) SEQPROF_CASE(8) SEQPROF_CASE(12) SEQPROF_CASE(16) SEQPROF_CASE(20) SEQPROF_CASE(24) SEQPROF_CASE(28) SEQPROF_CASE(32)
+        default: return cudaErrorInvalidValue;
+    }
+#undef SEQPROF_CASE
+}
 
 }  // namespace famsa
 
@@ -268,7 +315,7 @@ extern "C" int64_t famsa_seqprof_workspace(const int64_t* col_off_host, const in
     if (seqprof_check(col_off_host, seq_off_host, n_align, "famsa_seqprof_workspace") != FAMSA_OK) return -1;
     int64_t bytes = 0;
     for (int64_t b = 0; b < n_align; ++b)
-        bytes += (col_off_host[b + 1] - col_off_host[b] + 31) * 32 * lanes_j(seq_off_host[b + 1] - seq_off_host[b]);
+        bytes += dir_bytes_of(col_off_host[b + 1] - col_off_host[b], shape_of(seq_off_host[b + 1] - seq_off_host[b]));
     return bytes + n_align;                                  // + one final-state byte per alignment
 }
 
@@ -292,14 +339,16 @@ extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off
         AlignDesc& d = desc[(size_t)b];
         d.cost_row0 = col_off_host[b]; d.seq0 = seq_off_host[b];
         d.n1 = (int32_t)(col_off_host[b + 1] - col_off_host[b]); d.n2 = (int32_t)(seq_off_host[b + 1] - seq_off_host[b]);
-        d.idx = (int32_t)b; d.j = lanes_j(d.n2);
-        d.dir0 = dir_bytes; dir_bytes += ((int64_t)d.n1 + 31) * 32 * d.j;   // n1 + 31 wavefront steps
+        const Shape sh = shape_of(d.n2);
+        d.idx = (int32_t)b; d.j = (int16_t)sh.j; d.seg = (int16_t)sh.seg;
+        d.dir0 = dir_bytes; dir_bytes += dir_bytes_of(d.n1, sh);            // n1 + seg - 1 wavefront steps
         d.path_end = col_off_host[b + 1] + seq_off_host[b + 1];
         order[(size_t)b] = b;
     }
     std::stable_sort(order.begin(), order.end(), [&](int64_t p, int64_t q) {
         const AlignDesc &a = desc[(size_t)p], &c = desc[(size_t)q];
-        return a.j != c.j ? a.j > c.j : a.n1 > c.n1;            // heaviest group first, lighter groups fill its tail
+        if (a.j != c.j) return a.j > c.j;                       // heaviest group first, lighter groups fill its tail
+        return a.seg != c.seg ? a.seg > c.seg : a.n1 > c.n1;
     });
     std::lock_guard<std::mutex> desc_lock(g_desc_mu);
     DescStage& stg = g_desc[g_desc_next]; g_desc_next ^= 1;
@@ -329,25 +378,9 @@ extern "C" int famsa_seqprof_align(const float* cost_dev, const int64_t* col_off
     int64_t g0 = 0;
     while (g0 < n_align) {
         int64_t g1 = g0;
-        while (g1 < n_align && sorted[(size_t)g1].j == sorted[(size_t)g0].j) ++g1;
-        const int n = (int)(g1 - g0);
-        const unsigned grid = (unsigned)((n + 3) / 4);       // 4 warps = 4 alignments per CTA
-#define SEQPROF_CASE(JJ) case JJ: le = cudaLaunchKernelEx(&cfg, seqprof_kernel<JJ>, (const AlignDesc*)(d_desc + g0), n, cost_dev, seq_dev, gaps_dev, \
-                                                          nseq_dev, score_dev, final_state, ws, want_dir); break;
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = RING_BYTES; cfg.stream = st;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[0].val.programmaticStreamSerializationAllowed = 1;
-        cfg.attrs = attr; cfg.numAttrs = 1;
-        cudaError_t le = cudaSuccess;
-        switch (sorted[(size_t)g0].j) {
-            SEQPROF_CASE(4) SEQPROF_CASE(8) SEQPROF_CASE(12) SEQPROF_CASE(16) SEQPROF_CASE(20) SEQPROF_CASE(24) SEQPROF_CASE(28)
-            default: le = cudaLaunchKernelEx(&cfg, seqprof_kernel<32>, (const AlignDesc*)(d_desc + g0), n, cost_dev, seq_dev, gaps_dev,
-                                             nseq_dev, score_dev, final_state, ws, want_dir); break;
-        }
-        FAMSA_CUDA(le);
-#undef SEQPROF_CASE
+        while (g1 < n_align && sorted[(size_t)g1].j == sorted[(size_t)g0].j && sorted[(size_t)g1].seg == sorted[(size_t)g0].seg) ++g1;
+        FAMSA_CUDA(launch_seqprof_group(sorted[(size_t)g0].seg, sorted[(size_t)g0].j, d_desc + g0, (int)(g1 - g0), cost_dev, seq_dev, gaps_dev,
+                                        nseq_dev, score_dev, final_state, ws, want_dir, st));
         g0 = g1;
     }
     if (path_dev)
@@ -402,19 +435,19 @@ extern "C" int famsa_seqprof_scores_static(const float* cost_dev, const int64_t*
     }
     AlignDesc* d_desc = reinterpret_cast<AlignDesc*>(g_static_dev_ptr[device]);
     uint8_t* final_state = g_static_dev_ptr[device] + STATIC_DESC_BYTES;
-    // descriptors grouped by residues per lane, heaviest group first: a counting sort over the 8 classes into the static
+    // descriptors grouped by (lanes per alignment, residues per lane): a counting sort over the 16 classes into the static
     // host array (no heap allocation on this path)
-    int64_t start[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};                  // class c = 8 - J/4 (J = 32 first)
-    for (int64_t b = 0; b < n_align; ++b) start[8 - lanes_j(seq_off_host[b + 1] - seq_off_host[b]) / 4 + 1]++;
-    for (int c = 0; c < 8; ++c) start[c + 1] += start[c];
-    int64_t fill[8];
-    for (int c = 0; c < 8; ++c) fill[c] = start[c];
+    int64_t start[17] = {};                                          // 16 (seg, J) classes, see shape_class
+    for (int64_t b = 0; b < n_align; ++b) start[shape_class(shape_of(seq_off_host[b + 1] - seq_off_host[b])) + 1]++;
+    for (int c = 0; c < 16; ++c) start[c + 1] += start[c];
+    int64_t fill[16];
+    for (int c = 0; c < 16; ++c) fill[c] = start[c];
     for (int64_t b = 0; b < n_align; ++b) {
-        const int j = lanes_j(seq_off_host[b + 1] - seq_off_host[b]);
-        AlignDesc& d = g_static_host_desc[fill[8 - j / 4]++];
+        const Shape sh = shape_of(seq_off_host[b + 1] - seq_off_host[b]);
+        AlignDesc& d = g_static_host_desc[fill[shape_class(sh)]++];
         d.cost_row0 = col_off_host[b]; d.seq0 = seq_off_host[b];
         d.n1 = (int32_t)(col_off_host[b + 1] - col_off_host[b]); d.n2 = (int32_t)(seq_off_host[b + 1] - seq_off_host[b]);
-        d.idx = (int32_t)b; d.j = j;
+        d.idx = (int32_t)b; d.j = (int16_t)sh.j; d.seg = (int16_t)sh.seg;
         d.dir0 = 0; d.path_end = 0;                                  // no traceback in this variant
     }
     // The array keeps the previous call's contents.  Nothing in it has to start at zero: every descriptor and every
@@ -423,25 +456,11 @@ extern "C" int famsa_seqprof_scores_static(const float* cost_dev, const int64_t*
     FAMSA_CUDA(cudaMemsetAsync(final_state, 0, (size_t)n_align, st));
     // pageable source: the runtime has staged the bytes when the call returns, so the host array is free again
     FAMSA_CUDA(cudaMemcpyAsync(d_desc, g_static_host_desc, sizeof(AlignDesc) * (size_t)n_align, cudaMemcpyHostToDevice, st));
-    for (int c = 0; c < 8; ++c) {
-        const int64_t g0 = start[c];
+    for (int c = 0; c < 16; ++c) {
         const int n = (int)(start[c + 1] - start[c]);
         if (n == 0) continue;
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)((n + 3) / 4)); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = RING_BYTES; cfg.stream = st;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[0].val.programmaticStreamSerializationAllowed = 1;
-        cfg.attrs = attr; cfg.numAttrs = 1;
-        cudaError_t le = cudaSuccess;
-#define SEQPROF_STATIC_CASE(JJ) case JJ: le = cudaLaunchKernelEx(&cfg, seqprof_kernel<JJ>, (const AlignDesc*)(d_desc + g0), n, cost_dev, seq_dev, \
-                                                                 gaps_dev, nseq_dev, score_dev, final_state, (uint8_t*)nullptr, 0); break;
-        switch (32 - 4 * c) {
-            SEQPROF_STATIC_CASE(4) SEQPROF_STATIC_CASE(8) SEQPROF_STATIC_CASE(12) SEQPROF_STATIC_CASE(16)
-            SEQPROF_STATIC_CASE(20) SEQPROF_STATIC_CASE(24) SEQPROF_STATIC_CASE(28) SEQPROF_STATIC_CASE(32)
-        }
-#undef SEQPROF_STATIC_CASE
-        FAMSA_CUDA(le);
+        FAMSA_CUDA(launch_seqprof_group(c < 8 ? 32 : 16, 32 - 4 * (c & 7), d_desc + start[c], n, cost_dev, seq_dev, gaps_dev, nseq_dev, score_dev,
+                                        final_state, (uint8_t*)nullptr, 0, st));
     }
     return FAMSA_OK;
 }

@@ -38,7 +38,7 @@ def test_profile_exports_match_header(F):
         assert hasattr(L, name), name
     # host logic of the NEXT-4 boundary (no GPU needed)
     assert F.famsa_gap_scale(45) == 1.0
-    assert F.famsa_seqprof_workspace([0, 10, 30], [0, 100, 400]) == (10 + 31) * 32 * 4 + (20 + 31) * 32 * 12 + 2
+    assert F.famsa_seqprof_workspace([0, 10, 30], [0, 100, 400]) == (10 + 15) * 16 * 8 + (20 + 31) * 32 * 12 + 2
     with pytest.raises(F.FamsaError) as e:
         F.famsa_seqprof_workspace([0, 10], [0, 2000])         # more than 1024 residues
     assert e.value.code == F.FAMSA_ELENGTH
