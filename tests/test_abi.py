@@ -42,6 +42,15 @@ def test_profile_exports_match_header(F):
     with pytest.raises(F.FamsaError) as e:
         F.famsa_seqprof_workspace([0, 10], [0, 2000])         # more than 1024 residues
     assert e.value.code == F.FAMSA_ELENGTH
+    # argument validation happens before any CUDA call
+    off = np.arange(F.FAMSA_SEQPROF_STATIC_MAX + 2, dtype=np.int64)
+    assert L.famsa_seqprof_scores_static(None, off.ctypes.data, None, off.ctypes.data, None, None, F.FAMSA_SEQPROF_STATIC_MAX + 1, None, None) == F.FAMSA_ERANGE
+    assert b"FAMSA_SEQPROF_STATIC_MAX" in L.famsa_last_error()
+    assert L.famsa_seqprof_scores_static(None, off.ctypes.data, None, off.ctypes.data, None, None, 3, None, None) == F.FAMSA_EINVAL
+    assert L.famsa_seqprof_align(None, off.ctypes.data, None, off.ctypes.data, None, None, 3, None, None, None, None, None) == F.FAMSA_EINVAL
+    assert L.famsa_seqprof_align(None, None, None, None, None, None, 3, None, None, None, None, None) == F.FAMSA_EINVAL
+    assert L.famsa_seqprof_align(None, off.ctypes.data, None, off.ctypes.data, None, None, 0, None, None, None, None, None) == F.FAMSA_OK
+    assert L.famsa_profile_costs(None, None, 5, None, None) == F.FAMSA_EINVAL
 
 
 def test_rows_pairs(F):
