@@ -751,7 +751,7 @@ def run_seqprof(args, rank, world, local_rank):
                 "unit": "TIOP/s (ALU-pipe lane-instr)", "frac": cells * args.steps * alu_per_cell / (ms_rank * 1e-3) / peak["instr_per_s"],
                 "traffic": None, "algorithmic_instr_per_cell": alu_per_cell, "kernel": "famsa::seqprof_kernel<J>",
                 "peak_source": "famsa_alu_peak micro-kernel, measured in this run",
-                "note": "padding of n2 to 32 J lane slots, the 31-step skew of the wavefront and the traceback all count against the kernel"}
+                "note": "padding of n2 to SEG x J lane slots, the (SEG - 1)-step skew of the wavefront and the traceback all count against the kernel"}
     # e2e: pinned host inputs -> device, results back to pinned host, every step
     h_score = torch.empty(B, dtype=torch.float32).pin_memory(); h_path = torch.empty(path.numel(), dtype=torch.uint8).pin_memory()
     h_plen = torch.empty(B, dtype=torch.int32).pin_memory()

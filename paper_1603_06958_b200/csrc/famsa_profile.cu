@@ -243,7 +243,6 @@ __global__ void __launch_bounds__(128) seqprof_trace_kernel(const AlignDesc* __r
     }
 }
 
-// residues per lane: the smallest multiple of 4 with 32 J >= n2 (4 .. 32), so at most 127 of the 32 J lane slots idle
 // Pinned staging for the descriptors of a call: two buffers used alternately, each guarded by an event recorded
 // after its copy, so that a call neither synchronises the stream (a cudaMemcpyAsync from pageable memory would) nor
 // waits for more than the call before the previous one: consecutive batches overlap host preparation with the GPU.
